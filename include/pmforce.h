@@ -1,0 +1,171 @@
+/* pmforce.h -- C ABI of the B200-native particle-mesh force path of DISCO-DJ II (arXiv 2510.05206).
+ *
+ * Citations are "PAPER.md:<line>" plus the section / equation / table the line falls in; R<n> are the
+ * readings of the paper listed in DESIGN.md.
+ *
+ * Conventions (all calls)
+ *  - Every array pointer is a DEVICE pointer owned by the caller unless its name ends in `_host`.  The
+ *    library allocates only ctx-internal workspace (pm_create, and lazily on the first VJP / NUFFT call)
+ *    and frees it in pm_destroy.  Nothing is returned that the caller must free.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls enqueue work and
+ *    return; there is no hidden synchronisation except in pm_create / pm_destroy / pm_force_host /
+ *    pm_get_stage_ms and the first call that has to allocate lazily.
+ *  - Return value: 0 (PM_OK) or a negative pm_status.  Nothing aborts, throws or prints.  Asynchronous
+ *    CUDA faults surface on the next call that checks cudaGetLastError.
+ *  - Positions: fp32 [N,3] row-major (x,y,z per particle), any finite value (wrapped periodically into
+ *    [0, box), Eq. 2.1 "periodic").  Non-finite positions are the caller's responsibility.
+ *  - Meshes: fp32 [m][m][m] row-major, z fastest, dense (no padding); node j sits at r_j = j * box/m
+ *    (reading R3).  `m` is the PM mesh for pm_* calls and the fine grid
+ *    m_f = round(nufft_sigma * m) for nufft_* calls.  m and m_f must be multiples of 4 and >= 8.
+ *  - `shift`: host pointer to 3 doubles in length units (NULL = 0): the operator is evaluated with
+ *    W(r_j - X_i + s), i.e. particles displaced by -s (used for interlaced grids).
+ */
+#ifndef PMFORCE_H
+#define PMFORCE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pm_ctx pm_ctx; /* opaque: cuFFT plans, workspace, bin buffers, symbol tables */
+
+typedef enum pm_status {
+  PM_OK = 0,
+  PM_EINVAL = -1, /* bad parameter, NULL pointer, N > max_particles, unsupported option */
+  PM_ENOMEM = -2, /* device or host allocation failed */
+  PM_ECUDA = -3,  /* a CUDA runtime call or an earlier asynchronous kernel failed */
+  PM_ECUFFT = -4, /* a cuFFT call failed */
+  PM_ESTATE = -5  /* call not valid for this ctx (e.g. nufft_* on a ctx created with method = 0) */
+} pm_status;
+
+/* Plain-old-data, copied at pm_create.  Names follow Table 5. */
+typedef struct pm_params {
+  int32_t m;           /* mesh cells per dimension ("res_pm"); NUFFT: number of retained modes per dim   */
+  int32_t worder;      /* 2 CIC, 3 TSC, 4 PCS ("worder", Table 1)                        */
+  int32_t interlace;   /* 0 none; 1 two-grid Fourier-space combination; 2 two-grid force average (R1)     */
+  int32_t deconv_pow;  /* 0 none, 1 or 2: divide by W~(k)^deconv_pow ("deconvolve" = 2)      */
+  int32_t grad_order;  /* 0 exact i k; 2, 4, 6 finite-difference symbol (Table 2)        */
+  int32_t lap_order;   /* 0 exact -k^2; 2, 4, 6 finite-difference symbol (Table 2)                        */
+  int32_t method;      /* 0 PM (Sec. 2.5); 1 NUFFT                     */
+  int32_t nufft_width; /* ES-kernel width w in fine cells, 2..16; 0 = from nufft_eps (R10)                */
+  double box;          /* box size L > 0                                                                   */
+  double coeff;        /* C in Lap(phi) = C * delta, g = -grad(phi) (Eq. 2.1-2.2, R11)      */
+  double nufft_sigma;  /* upsampling factor sigma (5/4; BASELINE config 3: 2)                */
+  double nufft_eps;    /* requested NUFFT tolerance                                         */
+  int64_t max_particles; /* capacity of the binning workspace; N of every call must be <= this             */
+} pm_params;
+
+/* ---- lifetime ------------------------------------------------------------------------------------- */
+/* Validates p, builds cuFFT plans, symbol tables and workspace on the current CUDA device.  *out is set
+ * only on success.  Synchronises the device. */
+int pm_create(pm_ctx** out, const pm_params* p);
+int pm_destroy(pm_ctx* ctx); /* NULL is allowed */
+const char* pm_strerror(int code);
+const char* pm_last_error(const pm_ctx* ctx); /* detail of the last failure on this ctx ("" if none);
+                                                  NULL: why the last pm_create on this thread failed */
+
+/* Geometry the caller needs to allocate tensors. */
+int32_t pm_mesh_dim(const pm_ctx* ctx);        /* m   */
+int32_t pm_fine_dim(const pm_ctx* ctx);        /* m_f (0 unless method = 1) */
+int32_t pm_nufft_width(const pm_ctx* ctx);     /* w actually used (0 unless method = 1) */
+double pm_nufft_beta(const pm_ctx* ctx);       /* ES-kernel beta actually used */
+
+/* ---- a0: binning (the build's own step; north_star "sorted into cell tiles") ------------------------ */
+/* Sorts the N particles into mesh tiles (counting sort) and keeps the sorted records in the ctx.  After
+ * pm_bin, every call on this ctx that is given the SAME `pos` pointer and N reuses the records, so the
+ * caller must not change the positions at that address until the next pm_bin.  Calls given another
+ * pointer / N (or made without a prior pm_bin) bin internally first and drop the pinned records.
+ * For a method = 1 ctx the tiles are those of the fine grid. */
+int pm_bin(pm_ctx* ctx, const float* pos, int64_t N, void* stream);
+
+/* ---- a1: mass assignment, Eq. C.1, Table 1 kernels ----------------------------------- */
+/* mesh[j] += sum_i w_i W(r_j - X_i + s).  ACCUMULATES onto `mesh`: the caller zeroes it.
+ * w: [N] or NULL (all ones, "M_i = 1" PAPER.md:256). */
+int pm_assign(pm_ctx* ctx, const float* pos, const float* w, int64_t N, const double* shift,
+              float* mesh, void* stream);
+/* VJP of pm_assign (rule table): given mesh_cot [m^3],
+ *   pos_cot[i,b] = w_i sum_j mesh_cot[j] dW_j(X_i)/dX_i^b   (Eq. C.6, grad-W gather)  -- [N,3] or NULL
+ *   w_cot[i]     =     sum_j mesh_cot[j] W_j(X_i)           (Eq. C.8, scalar gather)  -- [N]   or NULL
+ * Both are overwritten.  (The cotangent of the input mesh is mesh_cot itself, Eq. C.4.) */
+int pm_assign_vjp(pm_ctx* ctx, const float* pos, const float* w, int64_t N, const double* shift,
+                  const float* mesh_cot, float* pos_cot, float* w_cot, void* stream);
+
+/* ---- a2-a4: FFT, Fourier-space kernel, inverse FFTs (Tables 1-2) ------------ */
+/* force_mesh[a] = IFFT( S_a * FFT(delta) ), S_a(n) = -Grad_a(n) coeff / Lap(n) / W~(n)^deconv_pow,
+ * S_a(0) = 0 (R7).  delta_mesh2 (grid shifted by half a cell) must be non-NULL iff interlace = 1; the
+ * spectra are then combined as 1/2 [d1 + e^{-ik.s} d2] (R1, R9).  force_mesh: host array of 3 device
+ * pointers, overwritten.  The inputs are not modified. */
+int pm_poisson_force(pm_ctx* ctx, const float* delta_mesh, const float* delta_mesh2,
+                     float* const force_mesh[3], void* stream);
+/* Transpose of pm_poisson_force: delta_cot = IFFT( sum_a conj(S_a) FFT(force_cot[a]) ) (overwritten);
+ * delta_cot2 receives the cotangent of the second grid iff interlace = 1 (else must be NULL). */
+int pm_poisson_force_vjp(pm_ctx* ctx, const float* const force_cot[3], float* delta_cot,
+                         float* delta_cot2, void* stream);
+
+/* ---- a5: gather, Eq. C.2 ------------------------------------------------------------- */
+/* out[i,a] = sum_j mesh[a][j] W(r_j - X_i + s), a < ncomp (1..3).  mesh: host array of ncomp device
+ * pointers.  out: [N,ncomp], overwritten, in the caller's particle order. */
+int pm_interp(pm_ctx* ctx, const float* const mesh[], int ncomp, const float* pos, int64_t N,
+              const double* shift, float* out, void* stream);
+/* VJP of pm_interp: given out_cot [N,ncomp],
+ *   mesh_cot[a][j] += sum_i out_cot[i,a] W_j(X_i)                         (Eq. C.10; ACCUMULATES) or NULL
+ *   pos_cot[i,b]    = sum_a out_cot[i,a] sum_j mesh[a][j] dW_j(X_i)/dX_i^b (Eq. C.12; overwritten) or NULL */
+int pm_interp_vjp(pm_ctx* ctx, const float* const mesh[], int ncomp, const float* pos, int64_t N,
+                  const double* shift, const float* out_cot, float* const mesh_cot[], float* pos_cot,
+                  void* stream);
+
+/* ---- a6-a8, a12: NUFFT path (method = 1), exponential-of-semicircle kernel ------- */
+/* fine[j] += sum_i c_i prod_a phi(2 (j_a - u_a)/w), u = X / (box/m_f); phi(z) = exp(beta (sqrt(1-z^2)-1)).
+ * ACCUMULATES.  c: [N] or NULL (ones). */
+int nufft_spread(pm_ctx* ctx, const float* pos, const float* c, int64_t N, float* fine, void* stream);
+int nufft_spread_vjp(pm_ctx* ctx, const float* pos, const float* c, int64_t N, const float* fine_cot,
+                     float* pos_cot, float* c_cot, void* stream);
+/* Spread grid -> three fine force grids: FFT, keep |n_a| < m/2 (R8), divide by phi_hat twice (R10,
+ * PAPER.md:262), Poisson + i k gradient, (coeff / n_particles) normalisation, zero-pad, inverse FFTs. */
+int nufft_poisson_force(pm_ctx* ctx, const float* fine, int64_t n_particles, float* const force_fine[3],
+                        void* stream);
+int nufft_poisson_force_vjp(pm_ctx* ctx, const float* const force_cot[3], int64_t n_particles,
+                            float* fine_cot, void* stream);
+/* out[i,a] = sum_j fine[a][j] prod_b phi(2 (j_b - u_b)/w)  (Eq. 2.19 through the grid). */
+int nufft_interp(pm_ctx* ctx, const float* const fine[], int ncomp, const float* pos, int64_t N,
+                 float* out, void* stream);
+int nufft_interp_vjp(pm_ctx* ctx, const float* const fine[], int ncomp, const float* pos, int64_t N,
+                     const float* out_cot, float* const fine_cot[], float* pos_cot, void* stream);
+
+/* ---- whole path ------------------------------------------------------------------------------------- */
+/* force[i,:] = A(X_i): a0-a5 (method 0: bin, assign (x2 if interlaced), R2C, k-space, 3 C2R, gather; the
+ * density contrast delta = (m^3/N) rho - 1 of Eq. 2.3 PAPER.md:92 is folded into the k-space kernel) or
+ * a0, a6-a8 (method 1).  force: [N,3], overwritten. */
+int pm_force(pm_ctx* ctx, const float* pos, int64_t N, float* force, void* stream);
+/* pos_cot = force_cot^T dA/dX (a9-a11; App. C).  Recomputes the forward meshes.
+ * force_cot: [N,3]; pos_cot: [N,3], overwritten. */
+int pm_force_vjp(pm_ctx* ctx, const float* pos, int64_t N, const float* force_cot, float* pos_cot,
+                 void* stream);
+/* Same as pm_force with HOST buffers: copies pos_host to the device, runs pm_force, copies the forces
+ * back and synchronises.  Pinned host memory gives asynchronous copies; pageable memory also works. */
+int pm_force_host(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream);
+
+/* ---- measurement ------------------------------------------------------------------------------------ */
+/* When enabled, pm_force / pm_force_vjp record CUDA events around each stage on the caller's stream. */
+int pm_set_profiling(pm_ctx* ctx, int enable);
+#define PM_STAGE_BIN 0
+#define PM_STAGE_ASSIGN 1
+#define PM_STAGE_FFT_FWD 2
+#define PM_STAGE_KSPACE 3
+#define PM_STAGE_FFT_INV 4
+#define PM_STAGE_INTERP 5
+#define PM_STAGE_VJP_SCATTER 6
+#define PM_STAGE_VJP_KSPACE 7 /* 3 R2C + transposed kernel + C2R */
+#define PM_STAGE_VJP_GATHER 8
+#define PM_NUM_STAGES 9
+/* Synchronises on the last profiled call and writes the duration in ms of each stage (0 if it did not
+ * run) to ms_host[0..n-1], n <= PM_NUM_STAGES.  launches_host (or NULL) receives how many kernels of
+ * this library (cuFFT's excluded) that call launched. */
+int pm_get_stage_ms(pm_ctx* ctx, float* ms_host, int n, int64_t* launches_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PMFORCE_H */

@@ -1,0 +1,63 @@
+// nufft_mesh.cu -- a6 / a8 / a12: spreading and interpolation with the exponential-of-semicircle kernel
+// (Eq. 2.18-2.19): instantiations of k_scatter / k_gather for one
+// kernel width.  Compiled once per supported width with -DES_W=<w>; nufft_dispatch.cu selects at run time.
+#include "pm_mesh_kernels.cuh"
+
+#ifndef ES_W
+#error "compile with -DES_W=<kernel width>"
+#endif
+
+namespace pmf {
+
+template <int W>
+int es_scatter_w(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[], cudaStream_t st);
+template <int W>
+int es_gather_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
+
+template <class T>
+static typename T::Params es_params(const Ctx* c) {
+  typename T::Params tp;
+  tp.frac[0] = tp.frac[1] = tp.frac[2] = 0u;
+  tp.beta = (float)c->nufft_beta;
+  return tp;
+}
+
+template <>
+int es_scatter_w<ES_W>(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[], cudaStream_t st) {
+  using T = ESTraits<ES_W>;
+  const typename T::Params tp = es_params<T>(c);
+  const int roll[3] = {0, 0, 0};
+  if (!wsrc) {
+    for (int a = 0; a < ncomp; ++a) PM_TRY((run_scatter<T, 1, false>(c, tp, roll, nullptr, 0, mesh + a, st)));
+    return PM_OK;
+  }
+  if (ncomp == 3) return run_scatter<T, 3, true>(c, tp, roll, wsrc, wstride, mesh, st);
+  for (int a = 0; a < ncomp; ++a) PM_TRY((run_scatter<T, 1, true>(c, tp, roll, wsrc + a, wstride, mesh + a, st)));
+  return PM_OK;
+}
+
+template <class T, int NCOMP, bool GRAD>
+static int go(Ctx* c, const GatherArgs& a, cudaStream_t st) {
+  constexpr size_t smem = sizeof(float) * (size_t)NCOMP * Geo<T>::PLANE;
+  if (smem > 200 * 1024) return fail(c, PM_EINVAL, "ES gather: %d meshes of width %d do not fit in shared memory", NCOMP, T::P);
+  const int roll[3] = {0, 0, 0};
+  return run_gather<T, NCOMP, GRAD>(c, es_params<T>(c), roll, a.mesh, a.cot, a.cstride, a.ncot, a.const_coef, a.wmul,
+                                    a.alpha, a.accumulate, a.out, st);
+}
+
+template <>
+int es_gather_w<ES_W>(Ctx* c, const GatherArgs& a, cudaStream_t st) {
+  using T = ESTraits<ES_W>;
+  switch (a.ncomp * 2 + (a.grad ? 1 : 0)) {
+    case 2: return go<T, 1, false>(c, a, st);
+    case 3: return go<T, 1, true>(c, a, st);
+    case 4: return go<T, 2, false>(c, a, st);
+    case 5: return go<T, 2, true>(c, a, st);
+    case 6: return go<T, 3, false>(c, a, st);
+    case 7: return go<T, 3, true>(c, a, st);
+    case 9: return go<T, 4, true>(c, a, st);
+  }
+  return fail(c, PM_EINVAL, "ES gather: unsupported ncomp = %d", a.ncomp);
+}
+
+}  // namespace pmf

@@ -1,0 +1,280 @@
+// pm_bin.cu -- a0: on-device counting sort of particles into mesh tiles (north_star: "Particles are
+// sorted into cell tiles with an on-device counting/Morton sort").  Not in the paper; the build's own step.
+//
+//   pass 1  k_count   : cell coordinate in fp64 from the fp32 position, tile histogram (warp-aggregated)
+//   scan    k_scan_*  : exclusive scans of the tile counts and of the per-tile work-item counts
+//   pass 2  k_permute : recompute the coordinate, claim a slot (warp-aggregated, order-preserving inside a
+//                       warp), store the record {ux, uy, uz, i} with tile-local fixed-point coordinates
+//   items   k_items   : work items (tile, begin, end) of at most CHUNK particles
+//
+// Algorithmic bytes: 12N (read) + 12N (read) + 16N (write); the tile arrays are O(ntiles).
+#include "pm_internal.cuh"
+
+namespace pmf {
+
+struct BinGeom {
+  int m, ntx, nty, ntz;
+  double inv_dx;  // m / box
+};
+
+// u = x * m/L in fp64, wrapped into [0, m).  (SURVEY 7 "hard parts": the fp32 product is not enough.)
+__device__ __forceinline__ double cell_coord(float x, const BinGeom& g) {
+  double u = (double)x * g.inv_dx;
+  const double dm = (double)g.m;
+  if (u < 0.0 || u >= dm) {
+    u -= dm * floor(u / dm);
+    if (!(u >= 0.0) || u >= dm) u = 0.0;
+  }
+  return u;
+}
+
+__device__ __forceinline__ uint32_t tile_and_local(float x, float y, float z, const BinGeom& g, uint32_t& fx,
+                                                   uint32_t& fy, uint32_t& fz) {
+  const double ux = cell_coord(x, g), uy = cell_coord(y, g), uz = cell_coord(z, g);
+  const int tx = (int)ux / TX, ty = (int)uy / TY, tz = (int)uz / TZ;
+  const double s = (double)REC_ONE;
+  // (u_local + REC_BIAS) * 2^REC_FRAC, clamped below the next tile so the integer part stays in-tile
+  fx = min((uint32_t)__double2ll_rn((ux - tx * TX + REC_BIAS) * s), (uint32_t)((TX + REC_BIAS) * REC_ONE - 1u));
+  fy = min((uint32_t)__double2ll_rn((uy - ty * TY + REC_BIAS) * s), (uint32_t)((TY + REC_BIAS) * REC_ONE - 1u));
+  fz = min((uint32_t)__double2ll_rn((uz - tz * TZ + REC_BIAS) * s), (uint32_t)((TZ + REC_BIAS) * REC_ONE - 1u));
+  return (uint32_t)((tx * g.nty + ty) * g.ntz + tz);
+}
+
+__device__ __forceinline__ uint32_t tile_only(float x, float y, float z, const BinGeom& g) {
+  const int tx = (int)cell_coord(x, g) / TX, ty = (int)cell_coord(y, g) / TY, tz = (int)cell_coord(z, g) / TZ;
+  return (uint32_t)((tx * g.nty + ty) * g.ntz + tz);
+}
+
+// Lanes of a warp that share `key` elect a leader which performs ONE atomic for the group; returns the
+// slot of this lane (leader's base + rank in lane order, so a coherent input keeps its order in a tile).
+__device__ __forceinline__ uint32_t warp_claim(uint32_t* counters, uint32_t key, bool valid) {
+  const unsigned lane = threadIdx.x & 31u;
+  const unsigned peers = __match_any_sync(0xffffffffu, valid ? key : 0xffffffffu);
+  const int leader = __ffs(peers) - 1;
+  uint32_t base = 0;
+  if (valid && (int)lane == leader) base = atomicAdd(&counters[key], (uint32_t)__popc(peers));
+  base = __shfl_sync(0xffffffffu, base, leader);
+  return base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+}
+
+// Four particles per thread, three coalesced float4 loads (north_star "coalesced float4 position loads").
+struct Quad {
+  float x[4], y[4], z[4];
+};
+__device__ __forceinline__ Quad load_quad(const float4* __restrict__ p4, int64_t q) {
+  const float4 a = __ldg(p4 + 3 * q), b = __ldg(p4 + 3 * q + 1), c = __ldg(p4 + 3 * q + 2);
+  Quad r;
+  r.x[0] = a.x; r.y[0] = a.y; r.z[0] = a.z;
+  r.x[1] = a.w; r.y[1] = b.x; r.z[1] = b.y;
+  r.x[2] = b.z; r.y[2] = b.w; r.z[2] = c.x;
+  r.x[3] = c.y; r.y[3] = c.z; r.z[3] = c.w;
+  return r;
+}
+
+template <bool PERMUTE>
+__global__ void __launch_bounds__(256) k_bin_pass(const float* __restrict__ pos, int64_t n, BinGeom g,
+                                                  uint32_t* __restrict__ counters,
+                                                  const uint32_t* __restrict__ tile_off,
+                                                  uint4* __restrict__ rec, int aligned) {
+  const int64_t nquad = aligned ? n / 4 : 0;
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  const int64_t t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const float4* p4 = reinterpret_cast<const float4*>(pos);
+  // vector body: every lane of a warp runs the same number of iterations (warp_claim is warp-wide)
+  const int64_t nq_round = (nquad + 31) / 32 * 32;
+  for (int64_t q = t0; q < nq_round; q += stride) {
+    const bool valid = q < nquad;
+    Quad pq;
+    if (valid) pq = load_quad(p4, q);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      uint32_t fx = 0, fy = 0, fz = 0, tile = 0;
+      if (valid) tile = PERMUTE ? tile_and_local(pq.x[k], pq.y[k], pq.z[k], g, fx, fy, fz)
+                                : tile_only(pq.x[k], pq.y[k], pq.z[k], g);
+      const uint32_t slot = warp_claim(counters, tile, valid);
+      if (PERMUTE && valid) rec[tile_off[tile] + slot] = make_uint4(fx, fy, fz, (uint32_t)(4 * q + k));
+    }
+  }
+  // scalar tail (and the whole array when pos is not 16-byte aligned)
+  const int64_t first = nquad * 4;
+  const int64_t rest = n - first;
+  const int64_t rest_round = (rest + 31) / 32 * 32;
+  for (int64_t j = t0; j < rest_round; j += stride) {
+    const bool valid = j < rest;
+    uint32_t fx = 0, fy = 0, fz = 0, tile = 0;
+    const int64_t i = first + j;
+    if (valid) {
+      const float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+      tile = PERMUTE ? tile_and_local(x, y, z, g, fx, fy, fz) : tile_only(x, y, z, g);
+    }
+    const uint32_t slot = warp_claim(counters, tile, valid);
+    if (PERMUTE && valid) rec[tile_off[tile] + slot] = make_uint4(fx, fy, fz, (uint32_t)i);
+  }
+}
+
+// ---- exclusive scan of (count, nchunks) over the tiles: reduce / scan-of-partials / rescan ----------
+constexpr int SCAN_T = 1024, SCAN_E = 4, SCAN_B = SCAN_T * SCAN_E;
+
+__device__ __forceinline__ uint32_t nchunks_of(uint32_t cnt) { return (cnt + CHUNK - 1) / CHUNK; }
+
+__device__ uint2 block_exclusive_scan(uint2 v, uint2* total) {  // blockDim.x == SCAN_T
+  __shared__ uint2 wsum[32];
+  const unsigned lane = threadIdx.x & 31u, wid = threadIdx.x >> 5;
+  uint2 incl = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t a = __shfl_up_sync(0xffffffffu, incl.x, d), b = __shfl_up_sync(0xffffffffu, incl.y, d);
+    if ((int)lane >= d) { incl.x += a; incl.y += b; }
+  }
+  if (lane == 31) wsum[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    uint2 w = wsum[lane];
+    uint2 wi = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t a = __shfl_up_sync(0xffffffffu, wi.x, d), b = __shfl_up_sync(0xffffffffu, wi.y, d);
+      if ((int)lane >= d) { wi.x += a; wi.y += b; }
+    }
+    wsum[lane] = make_uint2(wi.x - w.x, wi.y - w.y);
+    if (lane == 31 && total) *total = wi;
+  }
+  __syncthreads();
+  const uint2 off = wsum[wid];
+  __syncthreads();
+  return make_uint2(off.x + incl.x - v.x, off.y + incl.y - v.y);
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const uint32_t* __restrict__ cnt, int n,
+                                                        uint2* __restrict__ partial) {
+  __shared__ uint2 tot;
+  uint2 s = make_uint2(0, 0);
+  const int base = blockIdx.x * SCAN_B + threadIdx.x * SCAN_E;
+#pragma unroll
+  for (int e = 0; e < SCAN_E; ++e)
+    if (base + e < n) { const uint32_t c = cnt[base + e]; s.x += c; s.y += nchunks_of(c); }
+  block_exclusive_scan(s, &tot);
+  if (threadIdx.x == 0) partial[blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_partials(uint2* __restrict__ partial, int nb,
+                                                          uint32_t* __restrict__ tile_off,
+                                                          uint32_t* __restrict__ item_off, int ntiles,
+                                                          uint32_t* __restrict__ nitems) {
+  __shared__ uint2 tot;
+  uint2 carry = make_uint2(0, 0);
+  for (int b0 = 0; b0 < nb; b0 += SCAN_T) {
+    const int i = b0 + threadIdx.x;
+    const uint2 v = i < nb ? partial[i] : make_uint2(0, 0);
+    const uint2 ex = block_exclusive_scan(v, &tot);
+    if (i < nb) partial[i] = make_uint2(ex.x + carry.x, ex.y + carry.y);
+    carry.x += tot.x;
+    carry.y += tot.y;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    tile_off[ntiles] = carry.x;
+    item_off[ntiles] = carry.y;
+    *nitems = carry.y;
+  }
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_final(uint32_t* __restrict__ cnt, int n,
+                                                       const uint2* __restrict__ partial,
+                                                       uint32_t* __restrict__ tile_off,
+                                                       uint32_t* __restrict__ item_off) {
+  const int base = blockIdx.x * SCAN_B + threadIdx.x * SCAN_E;
+  uint32_t c[SCAN_E];
+  uint2 s = make_uint2(0, 0);
+#pragma unroll
+  for (int e = 0; e < SCAN_E; ++e) {
+    c[e] = base + e < n ? cnt[base + e] : 0u;
+    s.x += c[e];
+    s.y += nchunks_of(c[e]);
+  }
+  uint2 ex = block_exclusive_scan(s, nullptr);
+  const uint2 p = partial[blockIdx.x];
+  ex.x += p.x;
+  ex.y += p.y;
+#pragma unroll
+  for (int e = 0; e < SCAN_E; ++e)
+    if (base + e < n) {
+      tile_off[base + e] = ex.x;
+      item_off[base + e] = ex.y;
+      ex.x += c[e];
+      ex.y += nchunks_of(c[e]);
+      cnt[base + e] = 0u;  // becomes the cursor of pass 2
+    }
+}
+
+__global__ void __launch_bounds__(256) k_items(const uint32_t* __restrict__ tile_off,
+                                               const uint32_t* __restrict__ item_off, int ntiles,
+                                               WorkItem* __restrict__ items) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ntiles) return;
+  const uint32_t b = tile_off[t], e = tile_off[t + 1];
+  uint32_t it = item_off[t];
+  for (uint32_t s = b; s < e; s += CHUNK) {
+    WorkItem w;
+    w.tile = (uint32_t)t;
+    w.begin = s;
+    w.end = min(s + (uint32_t)CHUNK, e);
+    w.pad = 0;
+    items[it++] = w;
+  }
+}
+
+BinView bin_view(const Ctx* c) {
+  BinView v;
+  v.rec = c->rec;
+  v.items = c->items;
+  v.nitems = c->nitems;
+  v.m = c->mg;
+  v.ntx = c->ntx;
+  v.nty = c->nty;
+  v.ntz = c->ntz;
+  return v;
+}
+
+int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) {
+  if (!pos) return fail(c, PM_EINVAL, "pos is NULL");
+  if (N < 0 || N > c->cap) return fail(c, PM_EINVAL, "N = %lld outside [0, max_particles = %lld]", (long long)N, (long long)c->cap);
+  if (!pin && c->bin_valid && c->bin_pinned && c->bin_pos == pos && c->bin_n == N) return PM_OK;
+  c->bin_valid = false;
+  BinGeom g;
+  g.m = c->mg;
+  g.ntx = c->ntx;
+  g.nty = c->nty;
+  g.ntz = c->ntz;
+  g.inv_dx = (double)c->mg / c->p.box;
+  const int nt = c->ntiles;
+  const int nb = (nt + SCAN_B - 1) / SCAN_B;
+  uint2* partial = reinterpret_cast<uint2*>(c->scan_tmp);
+  PM_CUDA(c, cudaMemsetAsync(c->tile_cnt, 0, sizeof(uint32_t) * (size_t)nt, st));
+  const int aligned = ((reinterpret_cast<uintptr_t>(pos) & 15u) == 0) ? 1 : 0;
+  const int64_t work = aligned ? (N + 3) / 4 : N;
+  int grid = (int)((work + 255) / 256);
+  const int gmax = c->num_sms * 16;
+  if (grid > gmax) grid = gmax;
+  if (grid < 1) grid = 1;
+  if (N > 0) k_bin_pass<false><<<grid, 256, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, nullptr, aligned);
+  k_scan_reduce<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial);
+  k_scan_partials<<<1, SCAN_T, 0, st>>>(partial, nb, c->tile_off, c->item_off, nt, c->nitems);
+  k_scan_final<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, c->tile_off, c->item_off);
+  if (N > 0) k_bin_pass<true><<<grid, 256, 0, st>>>(pos, N, g, c->tile_cnt, c->tile_off, c->rec, aligned);
+  k_items<<<(nt + 255) / 256, 256, 0, st>>>(c->tile_off, c->item_off, nt, c->items);
+  count_launch(c, N > 0 ? 6 : 4);
+  PM_CUDA(c, cudaGetLastError());
+  c->bin_valid = true;
+  c->bin_pos = pos;
+  c->bin_n = N;
+  c->bin_pinned = pin;
+  return PM_OK;
+}
+
+}  // namespace pmf
+
+extern "C" int pm_bin(pm_ctx* ctx, const float* pos, int64_t N, void* stream) {
+  if (!ctx) return PM_EINVAL;
+  return pmf::ensure_bins(pmf::C(ctx), pos, N, (cudaStream_t)stream, true);
+}

@@ -1,0 +1,193 @@
+// pm_internal.cuh -- shared declarations of libpmforce (not part of the public ABI).
+//
+// Data layout in HBM:
+//   * meshes: dense fp32 [m][m][m], z fastest; half-complex spectra [m][m][m/2+1] float2.
+//   * sorted particle records: one uint4 per particle {ux, uy, uz, orig_index}; u* are tile-local cell
+//     coordinates in unsigned fixed point, value = (u_local + REC_BIAS) * 2^REC_FRAC, computed once in
+//     fp64 by the binning pass (the fp32 product x*(m/L) alone would cost 1e-5 of force accuracy).
+//   * tiles of TX x TY x TZ cells in z-fastest order; tile_off[ntiles+1]; work items (tile, begin, end)
+//     of at most CHUNK particles.
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/pmforce.h"
+
+namespace pmf {
+
+// ---- tile geometry ------------------------------------------------------------------------------
+constexpr int TX = 8, TY = 8, TZ = 16;  // cells per tile
+constexpr int BLOCK = 256;              // threads per CTA of the scatter / gather kernels
+constexpr int PPT = 8;                  // particles per thread and work item
+constexpr int CHUNK = BLOCK * PPT;      // max particles per work item
+constexpr int REC_FRAC = 26;            // fractional bits of a record coordinate
+constexpr int REC_BIAS = 2;             // cells added so that shifted / half-added values stay >= 0
+constexpr uint32_t REC_ONE = 1u << REC_FRAC;
+constexpr uint32_t REC_MASK = REC_ONE - 1u;
+
+struct WorkItem {
+  uint32_t tile, begin, end, pad;
+};
+
+// Everything a scatter / gather kernel needs to know about the grid and the binned particles.
+struct BinView {
+  const uint4* rec;
+  const WorkItem* items;
+  const uint32_t* nitems;
+  int m, ntx, nty, ntz;
+};
+
+enum { MAX_W = 16 };
+
+struct Ctx;
+
+// ---- error helpers ------------------------------------------------------------------------------
+int fail(Ctx* c, int code, const char* fmt, ...);
+#define PM_CUDA(c, expr)                                                                     \
+  do {                                                                                       \
+    cudaError_t e__ = (expr);                                                                \
+    if (e__ != cudaSuccess)                                                                  \
+      return pmf::fail((c), e__ == cudaErrorMemoryAllocation ? PM_ENOMEM : PM_ECUDA,         \
+                       "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__,    \
+                       __LINE__);                                                            \
+  } while (0)
+#define PM_CUFFT(c, expr)                                                                    \
+  do {                                                                                       \
+    cufftResult r__ = (expr);                                                                \
+    if (r__ != CUFFT_SUCCESS)                                                                \
+      return pmf::fail((c), r__ == CUFFT_ALLOC_FAILED ? PM_ENOMEM : PM_ECUFFT,               \
+                       "%s failed: cufftResult %d (%s:%d)", #expr, (int)r__, __FILE__,       \
+                       __LINE__);                                                            \
+  } while (0)
+#define PM_TRY(expr)             \
+  do {                           \
+    int rc__ = (expr);           \
+    if (rc__ != PM_OK) return rc__; \
+  } while (0)
+
+// ---- the context --------------------------------------------------------------------------------
+struct Ctx {
+  pm_params p;
+  int device;
+  int num_sms;
+  int mg;        // grid the particles are binned on: m (PM) or m_f (NUFFT)
+  int m_modes;   // NUFFT: retained modes per dim (= p.m); PM: = m
+  int64_t G;     // mg^3
+  int64_t Gh;    // mg^2 (mg/2+1)
+  int ntx, nty, ntz, ntiles;
+  int nufft_w;
+  double nufft_beta;
+
+  // symbol tables, fp64, length mg each (device)
+  double* tab_grad;   // D(theta)/Delta         (PM)   | k_a               (NUFFT)
+  double* tab_lap;    // l(theta)/Delta^2       (PM)   | k_a^2             (NUFFT)
+  double* tab_win;    // W~(n)^deconv_pow       (PM)   | phi_hat(n)^2, 0 = mode dropped (NUFFT)
+  double* tab_cos;    // interlace phase, real part (R9)
+  double* tab_sin;    // interlace phase, imaginary part
+
+  // binning workspace
+  int64_t cap;
+  uint4* rec;
+  uint32_t* tile_cnt;   // [ntiles]   histogram, then reused as cursor
+  uint32_t* tile_off;   // [ntiles+1]
+  uint32_t* item_off;   // [ntiles+1]
+  uint32_t* scan_tmp;   // [2 * nblocks_scan + 2]
+  WorkItem* items;      // [max_items]
+  uint32_t* nitems;     // device scalar
+  int64_t max_items;
+  const float* bin_pos; // pointer the records were built from
+  int64_t bin_n;
+  bool bin_pinned;      // built by an explicit pm_bin
+  bool bin_valid;
+
+  // FFT
+  cufftHandle plan_r2c, plan_c2r;
+  bool plans_ok;
+  void* fft_work;
+  size_t fft_work_bytes;
+
+  // meshes owned by the ctx (pm_force path)
+  float* rho[2];     // assignment targets (second: interlace = 1)
+  float2* dhat[2];   // their spectra
+  float2* ghat[3];   // force spectra
+  float* g[3];       // force meshes
+  float* gbar[3];    // VJP: scattered cotangents (lazy)
+  bool vjp_ready;
+
+  // host staging for pm_force_host
+  float* host_pos_dev;
+  float* host_force_dev;
+
+  // profiling
+  bool profiling;
+  cudaEvent_t ev[2 * PM_NUM_STAGES];
+  bool ev_used[PM_NUM_STAGES];
+  bool ev_ok;
+  int64_t launches;
+  cudaStream_t prof_stream;
+
+  char err[512];
+};
+
+inline Ctx* C(pm_ctx* c) { return reinterpret_cast<Ctx*>(c); }
+inline const Ctx* C(const pm_ctx* c) { return reinterpret_cast<const Ctx*>(c); }
+
+struct ShiftSplit {
+  int roll[3];       // integer cells
+  uint32_t frac[3];  // fractional part in [0,1) as REC_FRAC fixed point
+  bool shifted;      // any frac != 0
+};
+ShiftSplit split_shift(const Ctx* c, const double* shift);
+
+// ---- stage entry points (host side, defined in the .cu files) ------------------------------------
+int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin);
+BinView bin_view(const Ctx* c);
+
+// Scatter ncomp (1..3) fields.  Weight of particle i, component a: wsrc ? wsrc[i*wstride + a] : 1.
+int launch_scatter(Ctx* c, int order, const ShiftSplit& sh, int ncomp, const float* wsrc, int wstride,
+                   float* const mesh[], cudaStream_t st);
+// Gather.  grad = false: v[i*ncomp + a] = sum_j mesh[a][j] W.
+// grad = true : v[i*3 + b] = sum_a coef_a(i) sum_j mesh[a][j] dW/dX^b, with
+//   coef_a(i) = a < ncot ? cot[i*cstride + a] : const_coef * (wmul ? wmul[i] : 1).
+// out = alpha * v (+ out if accumulate).
+struct GatherArgs {
+  int ncomp;
+  const float* const* mesh;
+  bool grad;
+  const float* cot;
+  int cstride, ncot;
+  float const_coef;
+  const float* wmul;
+  float alpha;
+  bool accumulate;
+  float* out;
+};
+inline GatherArgs gather_values(int ncomp, const float* const* mesh, float* out, float alpha = 1.f,
+                                bool accumulate = false) {
+  GatherArgs a = {ncomp, mesh, false, nullptr, 0, 0, 0.f, nullptr, alpha, accumulate, out};
+  return a;
+}
+int launch_gather(Ctx* c, int order, const ShiftSplit& sh, const GatherArgs& a, cudaStream_t st);
+
+// NUFFT spreading / interpolation with the ES kernel (same conventions).
+int launch_es_scatter(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[],
+                      cudaStream_t st);
+int launch_es_gather(Ctx* c, const GatherArgs& a, cudaStream_t st);
+
+// k-space kernels.
+int launch_kspace_forward(Ctx* c, const float2* d1, const float2* d2, float2* const ghat[3],
+                          double coeff_eff, cudaStream_t st);
+int launch_kspace_transpose(Ctx* c, const float2* const gh[3], float2* q1, float2* q2,
+                            double coeff_eff, cudaStream_t st);
+int fft_r2c(Ctx* c, const float* in, float2* out, cudaStream_t st);
+int fft_c2r(Ctx* c, float2* in, float* out, cudaStream_t st);
+
+// profiling helpers
+void stage_begin(Ctx* c, int stage, cudaStream_t st);
+void stage_end(Ctx* c, int stage, cudaStream_t st);
+inline void count_launch(Ctx* c, int n = 1) { c->launches += n; }
+
+}  // namespace pmf

@@ -1,0 +1,226 @@
+"""GPU parity of the whole path (pm_force / pm_force_vjp, PM and NUFFT) against the fp64 oracle on the
+BASELINE.json configurations (full size where the oracle finishes in seconds, reduced otherwise), plus the
+invariants that hold at any size.  Bars (BASELINE.json north_star): relative L2 force error <= 1e-5
+(CIC / TSC PM; PCS held to the same), <= 10 eps for the NUFFT path, VJPs <= 1e-5 relative.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import nufft_oracle as no
+from oracle import pm_oracle as po
+from pm_inputs import generators as gen
+
+pytestmark = pytest.mark.gpu
+
+FORCE_TOL = 1e-5
+VJP_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def pm():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2510_05206_b200 as pm_
+
+    return pm_
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def params_of(pm, c, n, **over):
+    kw = dict(m=c["m"], box=c["box"], max_particles=n, worder=c.get("worder", 2), interlace=c.get("interlace", 0),
+              deconv_pow=c.get("deconv_pow", 2), grad_order=c.get("grad_order", 0), lap_order=c.get("lap_order", 0))
+    kw.update(over)
+    return pm.PMParams(**kw)
+
+
+def oracle_kw(c, **over):
+    kw = dict(worder=c.get("worder", 2), interlace=c.get("interlace", 0), grad_order=c.get("grad_order", 0),
+              lap_order=c.get("lap_order", 0), deconv_pow=c.get("deconv_pow", 2))
+    kw.update(over)
+    return kw
+
+
+def gpu_force(pm, params, pos):
+    ctx = pm.pm_create(params)
+    f = torch.empty(pos.shape[0], 3, device="cuda")
+    pm.pm_force(ctx, dev(pos), f)
+    out = f.cpu().numpy()
+    pm.pm_destroy(ctx)
+    return out
+
+
+def gpu_force_vjp(pm, params, pos, lam):
+    ctx = pm.pm_create(params)
+    xb = torch.empty(pos.shape[0], 3, device="cuda")
+    pm.pm_force_vjp(ctx, dev(pos), dev(lam), xb)
+    out = xb.cpu().numpy()
+    pm.pm_destroy(ctx)
+    return out
+
+
+# name, n_p (None = full size), shuffle
+FORCE_CASES = [("cfg0", None, False), ("cfg0", None, True), ("cfg1", 64, False), ("cfg1", None, False),
+               ("cfg2", 64, False), ("cfg4", 64, False), ("cfg4", 64, True), ("headline", 64, False)]
+
+
+@pytest.mark.parametrize("name,n_p,shuffle", FORCE_CASES)
+def test_force_parity_configs(pm, name, n_p, shuffle):
+    pos, c = gen.make_config_positions(name, n_p=n_p, shuffle=shuffle)
+    f = gpu_force(pm, params_of(pm, c, pos.shape[0]), pos)
+    ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
+    err = rel_l2(f, ref)
+    assert err <= FORCE_TOL, err
+    if c.get("interlace", 0) != 1:  # momentum conservation (same W for assign and gather); not for R1 mode 1
+        assert np.abs(f.astype(np.float64).sum(axis=0)).max() <= 2e-6 * np.abs(f).sum()
+
+
+@pytest.mark.parametrize("worder", [2, 3, 4])
+@pytest.mark.parametrize("interlace", [0, 1, 2])
+def test_force_parity_kernels_and_interlacing(pm, worder, interlace):
+    pos, c = gen.make_config_positions("cfg1", n_p=48)
+    c = dict(c, worder=worder, interlace=interlace)
+    f = gpu_force(pm, params_of(pm, c, pos.shape[0]), pos)
+    ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
+    assert rel_l2(f, ref) <= FORCE_TOL
+
+
+def test_zero_force_on_lattice(pm):
+    """Uniform lattice => zero force (R7), m = n_p and m = 2 n_p."""
+    for m in (32, 64):
+        pos = gen.uniform_lattice(32, 100.0, offset=0.3)
+        for worder in (2, 3, 4):
+            f = gpu_force(pm, pm.PMParams(m=m, box=100.0, max_particles=pos.shape[0], worder=worder, grad_order=4), pos)
+            # compare with the force scale of an rms-1-cell displaced lattice (~ box/m * coeff)
+            assert np.abs(f).max() <= 1e-5 * (100.0 / m)
+
+
+VJP_CASES = [("cfg1", 48, 1), ("cfg1", 48, 0), ("cfg1", 48, 2), ("cfg4", 48, 0), ("cfg0", None, 0)]
+
+
+@pytest.mark.parametrize("name,n_p,interlace", VJP_CASES)
+def test_force_vjp_parity(pm, name, n_p, interlace):
+    pos, c = gen.make_config_positions(name, n_p=n_p)
+    c = dict(c, interlace=interlace)
+    lam = gen.gaussian_cotangent(pos.shape[0], c.get("cot_seed", 2000))
+    xb = gpu_force_vjp(pm, params_of(pm, c, pos.shape[0]), pos, lam)
+    ref = po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c))
+    err = rel_l2(xb, ref)
+    assert err <= VJP_TOL, err
+
+
+def test_force_vjp_parity_cfg1_full(pm):
+    """BASELINE config 1 at full size: N = 128^3, TSC, two-grid interlacing, forward + VJP."""
+    pos, c = gen.make_config_positions("cfg1")
+    lam = gen.gaussian_cotangent(pos.shape[0], c["cot_seed"])
+    xb = gpu_force_vjp(pm, params_of(pm, c, pos.shape[0]), pos, lam)
+    ref = po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c))
+    assert rel_l2(xb, ref) <= VJP_TOL
+
+
+# ---- NUFFT path -----------------------------------------------------------------------------------------
+def nufft_params(pm, m, box, n, sigma=2.0, eps=1e-6, width=0):
+    return pm.PMParams(m=m, box=box, max_particles=n, method=1, nufft_sigma=sigma, nufft_eps=eps, nufft_width=width,
+                       grad_order=0, lap_order=0)
+
+
+@pytest.mark.parametrize("width", [4, 5, 6, 7, 8])
+def test_nufft_stage_parity(pm, width):
+    m, box = 20, 50.0
+    pos = np.concatenate([gen.uniform_random(15000, box, 61), gen.lattice_displaced(16, 40, box, 2.0, 62)])
+    n = pos.shape[0]
+    ctx = pm.pm_create(nufft_params(pm, m, box, n, width=width))
+    mf, w, beta = ctx.mg, ctx.nufft_width, ctx.nufft_beta
+    assert (mf, w) == (40, width)
+    assert abs(beta - no.es_params(1e-6, 2.0, width)[1]) < 1e-12
+    c = np.random.default_rng(9).standard_normal(n).astype(np.float32)
+    fine = torch.zeros(mf, mf, mf, device="cuda")
+    pm.nufft_spread(ctx, dev(pos), dev(c), fine)
+    ref = no.es_spread(pos, mf, box, w, beta, weights=c)
+    assert rel_l2(fine.cpu().numpy(), ref) <= 2e-6
+    meshes = gen.random_mesh(mf, 17, 3)
+    out = torch.empty(n, 3, device="cuda")
+    pm.nufft_interp(ctx, [dev(meshes[a]) for a in range(3)], dev(pos), out)
+    refi = np.stack([no.es_interp(meshes[a], pos, box, w, beta) for a in range(3)], axis=1)
+    assert rel_l2(out.cpu().numpy(), refi) <= 2e-6
+    # VJP pieces: grad gather (spread w.r.t. positions) and value gather (w.r.t. strengths)
+    pc = torch.empty(n, 3, device="cuda")
+    cc = torch.empty(n, device="cuda")
+    pm.nufft_spread_vjp(ctx, dev(pos), dev(c), dev(meshes[0]), pos_cot=pc, c_cot=cc)
+    refp = np.stack([c * no.es_interp(meshes[0], pos, box, w, beta, deriv_axis=b) for b in range(3)], axis=1)
+    assert rel_l2(cc.cpu().numpy(), refi[:, 0]) <= 2e-6
+    assert rel_l2(pc.cpu().numpy(), refp) <= 5e-6
+    pm.pm_destroy(ctx)
+
+
+def test_nufft_kspace_parity(pm):
+    m, box, n = 16, 30.0, 1000
+    ctx = pm.pm_create(nufft_params(pm, m, box, n))
+    mf, w, beta = ctx.mg, ctx.nufft_width, ctx.nufft_beta
+    fine = gen.random_mesh(mf, 19)[0]
+    g = [torch.empty(mf, mf, mf, device="cuda") for _ in range(3)]
+    pm.nufft_poisson_force(ctx, dev(fine), n, g)
+    ref = no.nufft_kspace(fine, m, box, n, w, beta)
+    for a in range(3):
+        assert rel_l2(g[a].cpu().numpy(), ref[a]) <= 3e-6
+    cot = gen.random_mesh(mf, 20, 3)
+    fc = torch.empty(mf, mf, mf, device="cuda")
+    pm.nufft_poisson_force_vjp(ctx, [dev(cot[a]) for a in range(3)], n, fc)
+    refv = no.nufft_kspace_vjp([cot[a] for a in range(3)], m, box, n, w, beta)
+    assert rel_l2(fc.cpu().numpy(), refv) <= 3e-6
+    pm.pm_destroy(ctx)
+
+
+def test_nufft_force_vs_bruteforce_definition(pm):
+    """The GPU NUFFT force against the brute-force non-uniform DFT (Eq. 2.18-2.19), eps = 1e-6 -> 1e-5."""
+    m, box = 12, 30.0
+    pos = gen.uniform_random(700, box, 63)
+    f = gpu_force(pm, nufft_params(pm, m, box, pos.shape[0]), pos)
+    ref = no.nudft_force_bruteforce(pos, m, box)
+    assert rel_l2(f, ref) <= 1e-5
+
+
+@pytest.mark.parametrize("sigma,eps,width", [(2.0, 1e-6, 0), (1.25, 1e-4, 0), (2.0, 1e-3, 0), (1.25, 0.5, 5)])
+def test_nufft_force_parity(pm, sigma, eps, width):
+    """cfg3 at reduced size (n_p = 48, 48 modes, fine grid 96) and other (sigma, w) pairs, incl. the paper's
+    own default sigma = 5/4, w = 5.  GPU vs the oracle's ES-kernel NUFFT with the same (w, beta)."""
+    pos, c = gen.make_config_positions("cfg3", n_p=48)
+    f = gpu_force(pm, nufft_params(pm, c["m"], c["box"], pos.shape[0], sigma=sigma, eps=eps, width=width), pos)
+    ref = no.nufft_force(pos, c["m"], c["box"], sigma=sigma, eps=eps, width=width)
+    assert rel_l2(f, ref) <= 1e-5
+
+
+def test_nufft_force_vjp_parity(pm):
+    pos, c = gen.make_config_positions("cfg3", n_p=32)
+    lam = gen.gaussian_cotangent(pos.shape[0], 2003)
+    xb = gpu_force_vjp(pm, nufft_params(pm, c["m"], c["box"], pos.shape[0]), pos, lam)
+    ref = no.nufft_force_vjp(pos, lam, c["m"], c["box"])
+    assert rel_l2(xb, ref) <= VJP_TOL
+
+
+def test_pm_force_host_matches_device(pm):
+    pos, c = gen.make_config_positions("cfg0")
+    ctx = pm.pm_create(params_of(pm, c, pos.shape[0]))
+    f_dev = torch.empty(pos.shape[0], 3, device="cuda")
+    pm.pm_force(ctx, dev(pos), f_dev)
+    ph = torch.from_numpy(pos).pin_memory()
+    fh = torch.empty(pos.shape[0], 3).pin_memory()
+    pm.pm_force_host(ctx, ph, fh)
+    ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
+    assert rel_l2(fh.numpy(), ref) <= FORCE_TOL
+    assert rel_l2(fh.numpy(), f_dev.cpu().numpy()) <= 2e-6  # atomics: not bitwise
+    pm.pm_set_profiling(ctx, True)
+    pm.pm_force(ctx, dev(pos), f_dev)
+    ms, launches = pm.pm_get_stage_ms(ctx)
+    assert launches >= 8 and ms["assign"] > 0 and ms["interp"] > 0
+    pm.pm_destroy(ctx)

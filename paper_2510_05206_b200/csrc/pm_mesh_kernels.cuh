@@ -22,6 +22,8 @@ struct PMTraits {
   static constexpr int P = ORDER;
   static constexpr int HLO = (ORDER == 2 ? 0 : 1) + (SHIFTED ? 1 : 0);
   static constexpr int HHI = (ORDER == 2 ? 1 : 2);
+  // largest value of the 3-D kernel: W(0)^3 = 1 (CIC), (3/4)^3 (TSC), (2/3)^3 (PCS)
+  static constexpr float WMAX3 = ORDER == 2 ? 1.0f : (ORDER == 3 ? 0.421875f : 0.2962963f);
   struct Params {
     uint32_t frac[3];
   };
@@ -69,6 +71,7 @@ struct ESTraits {
   static constexpr bool ODD = (W & 1) != 0;
   static constexpr int HLO = ODD ? (W - 1) / 2 : W / 2 - 1;
   static constexpr int HHI = ODD ? (W + 1) / 2 : W / 2;
+  static constexpr float WMAX3 = 1.0f;  // phi(0) = 1
   struct Params {
     uint32_t frac[3];  // unused (no shift), kept for a uniform interface
     float beta;
@@ -158,7 +161,7 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
   using G = Geo<T>;
   constexpr int P = T::P;
   extern __shared__ __align__(16) int s_acc[];
-  __shared__ float s_red[BLOCK / 32];
+  __shared__ float s_red[(BLOCK / 32) * NCOMP];
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
@@ -171,7 +174,9 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
     // particles of this item -> registers
     uint4 r[PPT];
     float wv[PPT][NCOMP];
-    float wmax = 0.0f;
+    float wabs[NCOMP];
+#pragma unroll
+    for (int a = 0; a < NCOMP; ++a) wabs[a] = 0.0f;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
       const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
@@ -180,34 +185,51 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
 #pragma unroll
         for (int a = 0; a < NCOMP; ++a) {
           wv[k][a] = WEIGHTED ? __ldg(wsrc + (size_t)r[k].w * wstride + a) : 1.0f;
-          wmax = fmaxf(wmax, fabsf(wv[k][a]));
+          wabs[a] += fabsf(wv[k][a]);
         }
       }
     }
     for (int j = tid; j < NCOMP * G::PLANE / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
 
-    // fixed-point scale 2^sexp: n * max|w| * scale (+ rounding) stays inside 32 bits
-    int sexp;
+    // Fixed-point scale 2^sexp per component.  No node can receive more than B = WMAX3 * sum_i |w_i|
+    // (WMAX3 = largest 3-D kernel value), so B * scale <= 2^30 (signed) / 2^31 (unit weights, unsigned)
+    // plus n/2 of rounding never overflows 32 bits.
+    float scale[NCOMP], inv_scale[NCOMP];
     if (WEIGHTED) {
 #pragma unroll
-      for (int d = 16; d > 0; d >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(0xffffffffu, wmax, d));
-      if ((tid & 31) == 0) s_red[tid >> 5] = wmax;
-      __syncthreads();
-      float bm = 0.0f;
+      for (int a = 0; a < NCOMP; ++a) {
 #pragma unroll
-      for (int j = 0; j < BLOCK / 32; ++j) bm = fmaxf(bm, s_red[j]);
-      const float bound = (float)n * bm;
+        for (int d = 16; d > 0; d >>= 1) wabs[a] += __shfl_xor_sync(0xffffffffu, wabs[a], d);
+        if ((tid & 31) == 0) s_red[(tid >> 5) * NCOMP + a] = wabs[a];
+      }
+      __syncthreads();
+#pragma unroll
+      for (int a = 0; a < NCOMP; ++a) {
+        float tot = 0.0f;
+#pragma unroll
+        for (int j = 0; j < BLOCK / 32; ++j) tot += s_red[j * NCOMP + a];
+        const float bound = tot * (T::WMAX3 * 1.0001f);
+        int e = 0;
+        const float f = frexpf(bound, &e);
+        const int cl = (f == 0.5f) ? e - 1 : e;  // ceil(log2(bound))
+        int sexp = (bound > 0.0f && bound < 3.0e38f) ? 30 - cl : 0;
+        sexp = max(-100, min(100, sexp));
+        scale[a] = pow2i(sexp);
+        inv_scale[a] = pow2i(-sexp);
+      }
+    } else {
+      const float bound = (float)n * T::WMAX3;
       int e = 0;
       const float f = frexpf(bound, &e);
-      const int cl = (f == 0.5f) ? e - 1 : e;  // ceil(log2(bound))
-      sexp = bound > 0.0f ? 30 - cl : 0;
-      sexp = max(-100, min(100, sexp));
-    } else {
-      const int cl = n > 1 ? 32 - __clz((int)(n - 1)) : 0;  // ceil(log2(n))
-      sexp = 31 - cl;
+      const int cl = (f == 0.5f) ? e - 1 : e;
+      const int sexp = min(31, 31 - cl);
+#pragma unroll
+      for (int a = 0; a < NCOMP; ++a) {
+        scale[a] = pow2i(sexp);
+        inv_scale[a] = pow2i(-sexp);
+      }
       __syncthreads();
     }
-    const float scale = pow2i(sexp), inv_scale = pow2i(-sexp);
 
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
@@ -222,7 +244,7 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
         const int base = (sx * G::SY + sy) * G::SZ + sz;
         float ws[NCOMP];
 #pragma unroll
-        for (int a = 0; a < NCOMP; ++a) ws[a] = wv[k][a] * scale;
+        for (int a = 0; a < NCOMP; ++a) ws[a] = wv[k][a] * scale[a];
 #pragma unroll
         for (int a = 0; a < P; ++a)
 #pragma unroll
@@ -255,11 +277,16 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
       const int sy = row % G::SY, sx = row / G::SY;
       float4 f;
       if (WEIGHTED) {
-        f = make_float4(__int2float_rn(v.x) * inv_scale, __int2float_rn(v.y) * inv_scale,
-                        __int2float_rn(v.z) * inv_scale, __int2float_rn(v.w) * inv_scale);
+        float is = inv_scale[0];
+#pragma unroll
+        for (int a = 1; a < NCOMP; ++a)
+          if (comp == a) is = inv_scale[a];
+        f = make_float4(__int2float_rn(v.x) * is, __int2float_rn(v.y) * is, __int2float_rn(v.z) * is,
+                        __int2float_rn(v.w) * is);
       } else {
-        f = make_float4(__uint2float_rn((unsigned)v.x) * inv_scale, __uint2float_rn((unsigned)v.y) * inv_scale,
-                        __uint2float_rn((unsigned)v.z) * inv_scale, __uint2float_rn((unsigned)v.w) * inv_scale);
+        const float is = inv_scale[0];
+        f = make_float4(__uint2float_rn((unsigned)v.x) * is, __uint2float_rn((unsigned)v.y) * is,
+                        __uint2float_rn((unsigned)v.z) * is, __uint2float_rn((unsigned)v.w) * is);
       }
       const int gx = wrap(o.x0 - G::HLO + sx - roll.x, m), gy = wrap(o.y0 - G::HLO + sy - roll.y, m);
       const int gz = wrap(o.z0 - G::ZLO + 4 * q - roll.z, m);

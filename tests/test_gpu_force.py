@@ -12,6 +12,8 @@ from oracle import nufft_oracle as no
 from oracle import pm_oracle as po
 from pm_inputs import generators as gen
 
+from conftest import record_error
+
 pytestmark = pytest.mark.gpu
 
 FORCE_TOL = 1e-5
@@ -80,6 +82,7 @@ def test_force_parity_configs(pm, name, n_p, shuffle):
     f = gpu_force(pm, params_of(pm, c, pos.shape[0]), pos)
     ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
     err = rel_l2(f, ref)
+    record_error(f"force/{name}/n_p={n_p or c['n_p']}/shuffle={int(shuffle)}", err, FORCE_TOL)
     assert err <= FORCE_TOL, err
     if c.get("interlace", 0) != 1:  # momentum conservation (same W for assign and gather); not for R1 mode 1
         assert np.abs(f.astype(np.float64).sum(axis=0)).max() <= 2e-6 * np.abs(f).sum()
@@ -92,7 +95,9 @@ def test_force_parity_kernels_and_interlacing(pm, worder, interlace):
     c = dict(c, worder=worder, interlace=interlace)
     f = gpu_force(pm, params_of(pm, c, pos.shape[0]), pos)
     ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
-    assert rel_l2(f, ref) <= FORCE_TOL
+    err = rel_l2(f, ref)
+    record_error(f"force/cfg1-48/worder={worder}/interlace={interlace}", err, FORCE_TOL)
+    assert err <= FORCE_TOL, err
 
 
 def test_zero_force_on_lattice(pm):
@@ -116,6 +121,7 @@ def test_force_vjp_parity(pm, name, n_p, interlace):
     xb = gpu_force_vjp(pm, params_of(pm, c, pos.shape[0]), pos, lam)
     ref = po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c))
     err = rel_l2(xb, ref)
+    record_error(f"force_vjp/{name}/n_p={n_p or c['n_p']}/interlace={interlace}", err, VJP_TOL)
     assert err <= VJP_TOL, err
 
 
@@ -125,7 +131,9 @@ def test_force_vjp_parity_cfg1_full(pm):
     lam = gen.gaussian_cotangent(pos.shape[0], c["cot_seed"])
     xb = gpu_force_vjp(pm, params_of(pm, c, pos.shape[0]), pos, lam)
     ref = po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c))
-    assert rel_l2(xb, ref) <= VJP_TOL
+    err = rel_l2(xb, ref)
+    record_error("force_vjp/cfg1/full", err, VJP_TOL)
+    assert err <= VJP_TOL, err
 
 
 # ---- NUFFT path -----------------------------------------------------------------------------------------
@@ -187,7 +195,9 @@ def test_nufft_force_vs_bruteforce_definition(pm):
     pos = gen.uniform_random(700, box, 63)
     f = gpu_force(pm, nufft_params(pm, m, box, pos.shape[0]), pos)
     ref = no.nudft_force_bruteforce(pos, m, box)
-    assert rel_l2(f, ref) <= 1e-5
+    err = rel_l2(f, ref)
+    record_error("nufft_force/bruteforce-700", err, 1e-5)
+    assert err <= 1e-5, err
 
 
 @pytest.mark.parametrize("sigma,eps,width", [(2.0, 1e-6, 0), (1.25, 1e-4, 0), (2.0, 1e-3, 0), (1.25, 0.5, 5)])
@@ -197,7 +207,9 @@ def test_nufft_force_parity(pm, sigma, eps, width):
     pos, c = gen.make_config_positions("cfg3", n_p=48)
     f = gpu_force(pm, nufft_params(pm, c["m"], c["box"], pos.shape[0], sigma=sigma, eps=eps, width=width), pos)
     ref = no.nufft_force(pos, c["m"], c["box"], sigma=sigma, eps=eps, width=width)
-    assert rel_l2(f, ref) <= 1e-5
+    err = rel_l2(f, ref)
+    record_error(f"nufft_force/cfg3-48/sigma={sigma}/eps={eps}/w={width}", err, 1e-5)
+    assert err <= 1e-5, err
 
 
 def test_nufft_force_vjp_parity(pm):
@@ -205,7 +217,9 @@ def test_nufft_force_vjp_parity(pm):
     lam = gen.gaussian_cotangent(pos.shape[0], 2003)
     xb = gpu_force_vjp(pm, nufft_params(pm, c["m"], c["box"], pos.shape[0]), pos, lam)
     ref = no.nufft_force_vjp(pos, lam, c["m"], c["box"])
-    assert rel_l2(xb, ref) <= VJP_TOL
+    err = rel_l2(xb, ref)
+    record_error("nufft_force_vjp/cfg3-32", err, VJP_TOL)
+    assert err <= VJP_TOL, err
 
 
 def test_pm_force_host_matches_device(pm):

@@ -42,9 +42,13 @@ def _cuda_lib_dir(nvcc: str) -> str:
 
 
 def _units():
-    units = [(os.path.join(CSRC, s), os.path.join(OBJ, s[:-3] + ".o"), []) for s in SOURCES]
-    for w in ES_WIDTHS:
-        units.append((os.path.join(CSRC, "nufft_mesh.cu"), os.path.join(OBJ, f"nufft_mesh_w{w}.o"), [f"-DES_W={w}"]))
+    units = []
+    # widest kernels first: they take minutes to compile and should not start last
+    for w in sorted(ES_WIDTHS, reverse=True):
+        for part in (2, 1, 0):
+            units.append((os.path.join(CSRC, "nufft_mesh.cu"), os.path.join(OBJ, f"nufft_mesh_w{w}_p{part}.o"),
+                          [f"-DES_W={w}", f"-DES_PART={part}"]))
+    units += [(os.path.join(CSRC, s), os.path.join(OBJ, s[:-3] + ".o"), []) for s in SOURCES]
     return units
 
 

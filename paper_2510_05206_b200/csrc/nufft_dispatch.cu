@@ -1,4 +1,5 @@
-// nufft_dispatch.cu -- run-time selection of the ES-kernel width (one translation unit per width).
+// nufft_dispatch.cu -- run-time selection of the ES-kernel width (three translation units per width:
+// scatter, gather of values, grad-W gather; see build.py).
 #include "pm_internal.cuh"
 
 namespace pmf {
@@ -6,14 +7,18 @@ namespace pmf {
 template <int W>
 int es_scatter_w(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[], cudaStream_t st);
 template <int W>
-int es_gather_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
+int es_gather_values_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
+template <int W>
+int es_gather_grad_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
 
 #define ES_WIDTHS(X) X(4) X(5) X(6) X(7) X(8)
 #define DECL(W)                                                                                    \
   template <>                                                                                      \
   int es_scatter_w<W>(Ctx*, int, const float*, int, float* const[], cudaStream_t);                 \
   template <>                                                                                      \
-  int es_gather_w<W>(Ctx*, const GatherArgs&, cudaStream_t);
+  int es_gather_values_w<W>(Ctx*, const GatherArgs&, cudaStream_t);                                \
+  template <>                                                                                      \
+  int es_gather_grad_w<W>(Ctx*, const GatherArgs&, cudaStream_t);
 ES_WIDTHS(DECL)
 #undef DECL
 
@@ -33,7 +38,7 @@ int launch_es_gather(Ctx* c, const GatherArgs& a, cudaStream_t st) {
   if (c->bin_n == 0) return PM_OK;
   switch (c->nufft_w) {
 #define CASE(W) \
-  case W: return es_gather_w<W>(c, a, st);
+  case W: return a.grad ? es_gather_grad_w<W>(c, a, st) : es_gather_values_w<W>(c, a, st);
     ES_WIDTHS(CASE)
 #undef CASE
   }

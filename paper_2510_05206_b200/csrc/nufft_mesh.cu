@@ -3,8 +3,8 @@
 // kernel width.  Compiled once per supported width with -DES_W=<w>; nufft_dispatch.cu selects at run time.
 #include "pm_mesh_kernels.cuh"
 
-#ifndef ES_W
-#error "compile with -DES_W=<kernel width>"
+#if !defined(ES_W) || !defined(ES_PART)
+#error "compile with -DES_W=<kernel width> -DES_PART=<0 scatter | 1 gather of values | 2 grad-W gather>"
 #endif
 
 namespace pmf {
@@ -12,7 +12,9 @@ namespace pmf {
 template <int W>
 int es_scatter_w(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[], cudaStream_t st);
 template <int W>
-int es_gather_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
+int es_gather_values_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
+template <int W>
+int es_gather_grad_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
 
 template <class T>
 static typename T::Params es_params(const Ctx* c) {
@@ -22,6 +24,7 @@ static typename T::Params es_params(const Ctx* c) {
   return tp;
 }
 
+#if ES_PART == 0
 template <>
 int es_scatter_w<ES_W>(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[], cudaStream_t st) {
   using T = ESTraits<ES_W>;
@@ -36,28 +39,40 @@ int es_scatter_w<ES_W>(Ctx* c, int ncomp, const float* wsrc, int wstride, float*
   return PM_OK;
 }
 
+#else
 template <class T, int NCOMP, bool GRAD>
 static int go(Ctx* c, const GatherArgs& a, cudaStream_t st) {
-  constexpr size_t smem = sizeof(float) * (size_t)NCOMP * Geo<T>::PLANE;
+  constexpr size_t smem = sizeof(float) * (size_t)NCOMP * GeoG<T>::PLANE_PAD + 128;
   if (smem > 200 * 1024) return fail(c, PM_EINVAL, "ES gather: %d meshes of width %d do not fit in shared memory", NCOMP, T::P);
   const int roll[3] = {0, 0, 0};
   return run_gather<T, NCOMP, GRAD>(c, es_params<T>(c), roll, a.mesh, a.cot, a.cstride, a.ncot, a.const_coef, a.wmul,
                                     a.alpha, a.accumulate, a.out, st);
 }
 
+#if ES_PART == 1
 template <>
-int es_gather_w<ES_W>(Ctx* c, const GatherArgs& a, cudaStream_t st) {
+int es_gather_values_w<ES_W>(Ctx* c, const GatherArgs& a, cudaStream_t st) {
   using T = ESTraits<ES_W>;
-  switch (a.ncomp * 2 + (a.grad ? 1 : 0)) {
-    case 2: return go<T, 1, false>(c, a, st);
-    case 3: return go<T, 1, true>(c, a, st);
-    case 4: return go<T, 2, false>(c, a, st);
-    case 5: return go<T, 2, true>(c, a, st);
-    case 6: return go<T, 3, false>(c, a, st);
-    case 7: return go<T, 3, true>(c, a, st);
-    case 9: return go<T, 4, true>(c, a, st);
+  switch (a.ncomp) {
+    case 1: return go<T, 1, false>(c, a, st);
+    case 2: return go<T, 2, false>(c, a, st);
+    case 3: return go<T, 3, false>(c, a, st);
   }
   return fail(c, PM_EINVAL, "ES gather: unsupported ncomp = %d", a.ncomp);
 }
+#else
+template <>
+int es_gather_grad_w<ES_W>(Ctx* c, const GatherArgs& a, cudaStream_t st) {
+  using T = ESTraits<ES_W>;
+  switch (a.ncomp) {
+    case 1: return go<T, 1, true>(c, a, st);
+    case 2: return go<T, 2, true>(c, a, st);
+    case 3: return go<T, 3, true>(c, a, st);
+    case 4: return go<T, 4, true>(c, a, st);
+  }
+  return fail(c, PM_EINVAL, "ES gather: unsupported ncomp = %d", a.ncomp);
+}
+#endif
+#endif
 
 }  // namespace pmf

@@ -13,7 +13,7 @@
 namespace pmf {
 
 struct BinGeom {
-  int m, ntx, nty, ntz;
+  int m, ntx, nty, ntz, xbl;
   double inv_dx;  // m / box
 };
 
@@ -37,69 +37,74 @@ __device__ __forceinline__ uint32_t tile_and_local(float x, float y, float z, co
   fx = min((uint32_t)__double2ll_rn((ux - tx * TX + REC_BIAS) * s), (uint32_t)((TX + REC_BIAS) * REC_ONE - 1u));
   fy = min((uint32_t)__double2ll_rn((uy - ty * TY + REC_BIAS) * s), (uint32_t)((TY + REC_BIAS) * REC_ONE - 1u));
   fz = min((uint32_t)__double2ll_rn((uz - tz * TZ + REC_BIAS) * s), (uint32_t)((TZ + REC_BIAS) * REC_ONE - 1u));
-  return (uint32_t)((tx * g.nty + ty) * g.ntz + tz);
+  return tile_id(tx, ty, tz, g.nty, g.ntz, g.xbl);
 }
 
 __device__ __forceinline__ uint32_t tile_only(float x, float y, float z, const BinGeom& g) {
   const int tx = (int)cell_coord(x, g) / TX, ty = (int)cell_coord(y, g) / TY, tz = (int)cell_coord(z, g) / TZ;
-  return (uint32_t)((tx * g.nty + ty) * g.ntz + tz);
+  return tile_id(tx, ty, tz, g.nty, g.ntz, g.xbl);
 }
 
-// Lanes of a warp that share `key` elect a leader which performs ONE atomic for the group; returns the
-// slot of this lane (leader's base + rank in lane order, so a coherent input keeps its order in a tile).
+// The lanes of a warp hold 32 CONSECUTIVE particles.  Each run of equal keys elects its first lane, which
+// performs ONE atomic for the run; returns the slot of this lane (run base + rank in the run), so that a
+// coherent input (Lagrangian order) keeps its order inside a tile -- the scatter / gather kernels rely on
+// that for conflict-free shared-memory access.  Lanes with valid = false take no slot.
 __device__ __forceinline__ uint32_t warp_claim(uint32_t* counters, uint32_t key, bool valid) {
   const unsigned lane = threadIdx.x & 31u;
-  const unsigned peers = __match_any_sync(0xffffffffu, valid ? key : 0xffffffffu);
-  const int leader = __ffs(peers) - 1;
+  if (!valid) key = 0xffffffffu;
+  const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+  const unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || key != prev);
+  const unsigned le = heads & (0xffffffffu >> (31u - lane));   // heads at or below this lane
+  const int head = 31 - __clz(le);
+  const unsigned above = heads & ~(0xffffffffu >> (31u - lane));
+  const int next = above ? __ffs(above) - 1 : 32;
   uint32_t base = 0;
-  if (valid && (int)lane == leader) base = atomicAdd(&counters[key], (uint32_t)__popc(peers));
-  base = __shfl_sync(0xffffffffu, base, leader);
-  return base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+  if (valid && (int)lane == head) base = atomicAdd(&counters[key], (uint32_t)(next - (int)lane));
+  base = __shfl_sync(0xffffffffu, base, head);
+  return base + (lane - (unsigned)head);
 }
 
-// Four particles per thread, three coalesced float4 loads (north_star "coalesced float4 position loads").
-struct Quad {
-  float x[4], y[4], z[4];
-};
-__device__ __forceinline__ Quad load_quad(const float4* __restrict__ p4, int64_t q) {
-  const float4 a = __ldg(p4 + 3 * q), b = __ldg(p4 + 3 * q + 1), c = __ldg(p4 + 3 * q + 2);
-  Quad r;
-  r.x[0] = a.x; r.y[0] = a.y; r.z[0] = a.z;
-  r.x[1] = a.w; r.y[1] = b.x; r.z[1] = b.y;
-  r.x[2] = b.z; r.y[2] = b.w; r.z[2] = c.x;
-  r.x[3] = c.y; r.y[3] = c.z; r.z[3] = c.w;
-  return r;
-}
+constexpr int BIN_BLOCK = 256;
+constexpr int BIN_WARP_PART = 128;  // particles per warp and iteration (3 float4 per lane)
 
+// pass 1 (PERMUTE = false): tile histogram; pass 2 (PERMUTE = true): claim a slot, store the record.
+// Positions are read as coalesced float4 (north_star "coalesced float4 position loads") and transposed
+// through a warp-private shared-memory strip so that lane l handles particles 32k + l, k = 0..3.
 template <bool PERMUTE>
-__global__ void __launch_bounds__(256) k_bin_pass(const float* __restrict__ pos, int64_t n, BinGeom g,
-                                                  uint32_t* __restrict__ counters,
-                                                  const uint32_t* __restrict__ tile_off,
-                                                  uint4* __restrict__ rec, int aligned) {
-  const int64_t nquad = aligned ? n / 4 : 0;
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  const int64_t t0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict__ pos, int64_t n, BinGeom g,
+                                                        uint32_t* __restrict__ counters,
+                                                        const uint32_t* __restrict__ tile_off,
+                                                        uint4* __restrict__ rec, int aligned) {
+  __shared__ __align__(16) float s_strip[BIN_BLOCK / 32][BIN_WARP_PART * 3];
+  const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+  float* s = s_strip[warp];
+  const int64_t nchunk = aligned ? n / BIN_WARP_PART : 0;
+  const int64_t gwarp = (int64_t)blockIdx.x * (BIN_BLOCK / 32) + warp;
+  const int64_t nwarps = (int64_t)gridDim.x * (BIN_BLOCK / 32);
   const float4* p4 = reinterpret_cast<const float4*>(pos);
-  // vector body: every lane of a warp runs the same number of iterations (warp_claim is warp-wide)
-  const int64_t nq_round = (nquad + 31) / 32 * 32;
-  for (int64_t q = t0; q < nq_round; q += stride) {
-    const bool valid = q < nquad;
-    Quad pq;
-    if (valid) pq = load_quad(p4, q);
+  for (int64_t ch = gwarp; ch < nchunk; ch += nwarps) {
+    const float4* src = p4 + ch * (BIN_WARP_PART * 3 / 4);
+    const float4 a = __ldg(src + lane), b = __ldg(src + 32 + lane), c = __ldg(src + 64 + lane);
+    reinterpret_cast<float4*>(s)[lane] = a;
+    reinterpret_cast<float4*>(s)[32 + lane] = b;
+    reinterpret_cast<float4*>(s)[64 + lane] = c;
+    __syncwarp();
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      uint32_t fx = 0, fy = 0, fz = 0, tile = 0;
-      if (valid) tile = PERMUTE ? tile_and_local(pq.x[k], pq.y[k], pq.z[k], g, fx, fy, fz)
-                                : tile_only(pq.x[k], pq.y[k], pq.z[k], g);
-      const uint32_t slot = warp_claim(counters, tile, valid);
-      if (PERMUTE && valid) rec[tile_off[tile] + slot] = make_uint4(fx, fy, fz, (uint32_t)(4 * q + k));
+      const int j = 32 * k + (int)lane;
+      const float x = s[3 * j], y = s[3 * j + 1], z = s[3 * j + 2];
+      uint32_t fx = 0, fy = 0, fz = 0;
+      const uint32_t tile = PERMUTE ? tile_and_local(x, y, z, g, fx, fy, fz) : tile_only(x, y, z, g);
+      const uint32_t slot = warp_claim(counters, tile, true);
+      if (PERMUTE) rec[tile_off[tile] + slot] = make_uint4(fx, fy, fz, (uint32_t)(ch * BIN_WARP_PART + j));
     }
+    __syncwarp();
   }
-  // scalar tail (and the whole array when pos is not 16-byte aligned)
-  const int64_t first = nquad * 4;
+  // scalar tail (and the whole array when pos is not 16-byte aligned); whole warps stay in the loop
+  const int64_t first = nchunk * BIN_WARP_PART;
   const int64_t rest = n - first;
   const int64_t rest_round = (rest + 31) / 32 * 32;
-  for (int64_t j = t0; j < rest_round; j += stride) {
+  for (int64_t j = gwarp * 32 + lane; j < rest_round; j += nwarps * 32) {
     const bool valid = j < rest;
     uint32_t fx = 0, fy = 0, fz = 0, tile = 0;
     const int64_t i = first + j;
@@ -233,6 +238,7 @@ BinView bin_view(const Ctx* c) {
   v.ntx = c->ntx;
   v.nty = c->nty;
   v.ntz = c->ntz;
+  v.xbl = c->xbl;
   return v;
 }
 
@@ -246,22 +252,24 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   g.ntx = c->ntx;
   g.nty = c->nty;
   g.ntz = c->ntz;
+  g.xbl = c->xbl;
   g.inv_dx = (double)c->mg / c->p.box;
   const int nt = c->ntiles;
   const int nb = (nt + SCAN_B - 1) / SCAN_B;
   uint2* partial = reinterpret_cast<uint2*>(c->scan_tmp);
   PM_CUDA(c, cudaMemsetAsync(c->tile_cnt, 0, sizeof(uint32_t) * (size_t)nt, st));
   const int aligned = ((reinterpret_cast<uintptr_t>(pos) & 15u) == 0) ? 1 : 0;
-  const int64_t work = aligned ? (N + 3) / 4 : N;
-  int grid = (int)((work + 255) / 256);
-  const int gmax = c->num_sms * 16;
+  // persistent grid: resident CTAs per SM (register-limited) x SMs, capped by the work
+  const int64_t work = aligned ? (N + BIN_WARP_PART - 1) / BIN_WARP_PART : (N + 31) / 32;  // warp iterations
+  int grid = (int)((work + BIN_BLOCK / 32 - 1) / (BIN_BLOCK / 32));
+  const int gmax = c->num_sms * c->bin_occ;
   if (grid > gmax) grid = gmax;
   if (grid < 1) grid = 1;
-  if (N > 0) k_bin_pass<false><<<grid, 256, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, nullptr, aligned);
+  if (N > 0) k_bin_pass<false><<<grid, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, nullptr, aligned);
   k_scan_reduce<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial);
   k_scan_partials<<<1, SCAN_T, 0, st>>>(partial, nb, c->tile_off, c->item_off, nt, c->nitems);
   k_scan_final<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, c->tile_off, c->item_off);
-  if (N > 0) k_bin_pass<true><<<grid, 256, 0, st>>>(pos, N, g, c->tile_cnt, c->tile_off, c->rec, aligned);
+  if (N > 0) k_bin_pass<true><<<grid, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, c->tile_off, c->rec, aligned);
   k_items<<<(nt + 255) / 256, 256, 0, st>>>(c->tile_off, c->item_off, nt, c->items);
   count_launch(c, N > 0 ? 6 : 4);
   PM_CUDA(c, cudaGetLastError());
@@ -270,6 +278,14 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   c->bin_n = N;
   c->bin_pinned = pin;
   return PM_OK;
+}
+
+int bin_occupancy() {
+  int a = 0, b = 0;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_bin_pass<false>, BIN_BLOCK, 0);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_bin_pass<true>, BIN_BLOCK, 0);
+  const int o = a < b ? a : b;
+  return o < 1 ? 1 : o;
 }
 
 }  // namespace pmf

@@ -40,6 +40,36 @@ ShiftSplit split_shift(const Ctx* c, const double* shift) {
   return s;
 }
 
+// ---- TMA tensor maps -----------------------------------------------------------------------------------
+// cuTensorMapEncodeTiled is a driver-API call; it is fetched through the runtime so that the library does
+// not link against libcuda directly.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn g_encode_tiled = nullptr;
+
+int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMap* out) {
+  if (!g_encode_tiled) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    PM_CUDA(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return fail(c, PM_ECUDA, "cuTensorMapEncodeTiled not available");
+    g_encode_tiled = (EncodeTiledFn)fn;
+  }
+  if (!base || (reinterpret_cast<uintptr_t>(base) & 15u))
+    return fail(c, PM_EINVAL, "mesh pointers must be non-NULL and 16-byte aligned");
+  const cuuint64_t m = (cuuint64_t)c->mg;
+  const cuuint64_t dims[3] = {m, m, m};                                       // innermost (z) first
+  const cuuint64_t strides[2] = {m * sizeof(float), m * m * sizeof(float)};   // bytes, dims 1 and 2
+  const cuuint32_t box[3] = {(cuuint32_t)sz, (cuuint32_t)sy, (cuuint32_t)sx};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = g_encode_tiled(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides,
+                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(c, PM_ECUDA, "cuTensorMapEncodeTiled failed: CUresult %d (box %d x %d x %d)", (int)r, sx, sy, sz);
+  return PM_OK;
+}
+
 // ---- symbol tables (Table 1 Fourier column, Table 2; readings R4-R6, R9) ---------------------------
 static double sinc_pi(double x) {  // sin(pi x)/(pi x)
   if (x == 0.0) return 1.0;
@@ -196,6 +226,8 @@ static int build(Ctx* c) {
   c->nty = (mg + TY - 1) / TY;
   c->ntz = (mg + TZ - 1) / TZ;
   c->ntiles = c->ntx * c->nty * c->ntz;
+  c->bin_occ = bin_occupancy();
+  c->xbl = (c->ntx % 8 == 0) ? 3 : (c->ntx % 4 == 0) ? 2 : (c->ntx % 2 == 0) ? 1 : 0;
 
   // tables
   std::vector<double> a(mg), b(mg), w(mg), pc(mg, 1.0), ps(mg, 0.0);

@@ -8,6 +8,7 @@
 //   * tiles of TX x TY x TZ cells in z-fastest order; tile_off[ntiles+1]; work items (tile, begin, end)
 //     of at most CHUNK particles.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <stdint.h>
@@ -38,7 +39,15 @@ struct BinView {
   const WorkItem* items;
   const uint32_t* nitems;
   int m, ntx, nty, ntz;
+  int xbl;  // log2 of xb; tiles are numbered ((tx / xb * nty + ty) * xb + tx % xb) * ntz + tz, see tile_id()
 };
+
+// Tile numbering.  Work items are processed in tile order by ~1000 concurrently resident CTAs, so tiles
+// that share a halo should be close in that order for the halo to be served from L2.  z-neighbours are
+// adjacent, y-neighbours xb * ntz apart, x-neighbours ntz apart inside a block of xb tile columns.
+__host__ __device__ __forceinline__ uint32_t tile_id(int tx, int ty, int tz, int nty, int ntz, int xbl) {
+  return (uint32_t)((((((tx >> xbl) * nty + ty) << xbl) | (tx & ((1 << xbl) - 1))) * ntz) + tz);
+}
 
 enum { MAX_W = 16 };
 
@@ -77,7 +86,8 @@ struct Ctx {
   int m_modes;   // NUFFT: retained modes per dim (= p.m); PM: = m
   int64_t G;     // mg^3
   int64_t Gh;    // mg^2 (mg/2+1)
-  int ntx, nty, ntz, ntiles;
+  int ntx, nty, ntz, ntiles, xbl;
+  int bin_occ;   // resident CTAs per SM of the binning kernels
   int nufft_w;
   double nufft_beta;
 
@@ -145,6 +155,7 @@ ShiftSplit split_shift(const Ctx* c, const double* shift);
 // ---- stage entry points (host side, defined in the .cu files) ------------------------------------
 int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin);
 BinView bin_view(const Ctx* c);
+int bin_occupancy();
 
 // Scatter ncomp (1..3) fields.  Weight of particle i, component a: wsrc ? wsrc[i*wstride + a] : 1.
 int launch_scatter(Ctx* c, int order, const ShiftSplit& sh, int ncomp, const float* wsrc, int wstride,
@@ -171,6 +182,9 @@ inline GatherArgs gather_values(int ncomp, const float* const* mesh, float* out,
   return a;
 }
 int launch_gather(Ctx* c, int order, const ShiftSplit& sh, const GatherArgs& a, cudaStream_t st);
+// Tensor map of a dense fp32 [m][m][m] mesh (m = c->mg) with a box of sx * sy * sz elements, no swizzle,
+// out-of-bounds elements zero-filled.  base must be 16-byte aligned (PM_EINVAL otherwise).
+int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMap* out);
 
 // NUFFT spreading / interpolation with the ES kernel (same conventions).
 int launch_es_scatter(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[],

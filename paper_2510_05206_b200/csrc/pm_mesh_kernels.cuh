@@ -9,6 +9,8 @@
 //   gather:  the tile plus halo of 1..4 meshes is staged in shared memory, each particle then reads its
 //            P^3 nodes from there.
 #pragma once
+#include <cuda.h>
+
 #include "pm_internal.cuh"
 
 namespace pmf {
@@ -106,6 +108,9 @@ struct ESTraits {
   }
 };
 
+// Shared-memory tile geometry.  The z origin of a staged tile is 4-aligned (ZLO = HLO rounded up): the scatter
+// flushes with 16-byte vector reductions and a TMA box must start on a 16-byte boundary of the innermost
+// dimension (measured: an unaligned start coordinate raises "illegal instruction" on sm_100a).
 template <class T>
 struct Geo {
   static constexpr int P = T::P, HLO = T::HLO, HHI = T::HHI;
@@ -113,6 +118,15 @@ struct Geo {
   static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, SZ = TZ + ZLO + ZHI;
   static constexpr int PLANE = SX * SY * SZ;         // smem words per component
   static constexpr int NGROUP = SX * SY * (SZ / 4);  // float4 groups per component
+};
+template <class T>
+struct GeoG {
+  static constexpr int P = T::P, HLO = T::HLO, HHI = T::HHI;
+  static constexpr int ZLO = (HLO + 3) / 4 * 4;
+  static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, SZ = (ZLO + TZ + HHI + 3) / 4 * 4;
+  static constexpr int PLANE = SX * SY * SZ;             // box elements per component
+  static constexpr int PLANE_PAD = (PLANE + 31) / 32 * 32;  // TMA destinations are 128-byte aligned
+  static constexpr int NGROUP = SX * SY * (SZ / 4);
 };
 
 template <int N>
@@ -123,10 +137,18 @@ template <int N>
 struct CMeshPtrs {
   const float* p[N];
 };
+template <int N>
+struct TMapSet {
+  CUtensorMap m[N];
+};
 
-__device__ __forceinline__ int wrap(int v, int m) {
+__device__ __forceinline__ int wrap(int v, int m) {  // general (slow: integer division by a run-time m)
   v %= m;
   return v < 0 ? v + m : v;
+}
+__device__ __forceinline__ int wrap_up(int v, int m) {  // v >= 0, a few multiples of m at most
+  while (v >= m) v -= m;
+  return v;
 }
 
 __device__ __forceinline__ void red_add_v4(float* addr, float4 v) {
@@ -140,13 +162,15 @@ __device__ __forceinline__ float pow2i(int e) { return __int_as_float((e + 127) 
 struct TileOrigin {
   int x0, y0, z0;
 };
-__device__ __forceinline__ TileOrigin tile_origin(uint32_t tile, const BinView& bv) {
+__device__ __forceinline__ TileOrigin tile_origin(uint32_t tile, const BinView& bv) {  // inverse of tile_id()
   TileOrigin o;
   const int tz = (int)(tile % (uint32_t)bv.ntz);
-  const int r = (int)(tile / (uint32_t)bv.ntz);
+  int r = (int)(tile / (uint32_t)bv.ntz);
+  const int xl = r & ((1 << bv.xbl) - 1);
+  r >>= bv.xbl;
   o.z0 = tz * TZ;
   o.y0 = (r % bv.nty) * TY;
-  o.x0 = (r / bv.nty) * TX;
+  o.x0 = (((r / bv.nty) << bv.xbl) | xl) * TX;
   return o;
 }
 
@@ -154,6 +178,8 @@ __device__ __forceinline__ TileOrigin tile_origin(uint32_t tile, const BinView& 
 __device__ __forceinline__ uint32_t apply_shift(uint32_t rec, uint32_t frac) { return rec - frac; }
 
 // ---- K2 / K5: tile scatter ---------------------------------------------------------------------------
+// Persistent CTAs loop over work items.  The accumulator tile is zeroed once; every flush writes zeros
+// back, so a work item costs two barriers.  roll is in [0, m).
 template <class T, int NCOMP, bool WEIGHTED>
 __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Params tp, int3 roll,
                                                    const float* __restrict__ wsrc, int wstride,
@@ -165,6 +191,9 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
+
+  for (int j = tid; j < NCOMP * G::PLANE / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
+  __syncthreads();
 
   for (uint32_t it = blockIdx.x; it < nitems; it += gridDim.x) {
     const WorkItem wi = bv.items[it];
@@ -189,7 +218,6 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
         }
       }
     }
-    for (int j = tid; j < NCOMP * G::PLANE / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
 
     // Fixed-point scale 2^sexp per component.  No node can receive more than B = WMAX3 * sum_i |w_i|
     // (WMAX3 = largest 3-D kernel value), so B * scale <= 2^30 (signed) / 2^31 (unit weights, unsigned)
@@ -228,7 +256,6 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
         scale[a] = pow2i(sexp);
         inv_scale[a] = pow2i(-sexp);
       }
-      __syncthreads();
     }
 
 #pragma unroll
@@ -268,11 +295,16 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
     }
     __syncthreads();
 
-    // flush: vectorised global reductions along z (red.global.add.v4.f32), empty groups skipped
+    // flush: vectorised global reductions along z (red.global.add.v4.f32), empty groups skipped; the
+    // accumulators are zeroed on the way out.  bx/by/bz >= 0 so one conditional subtraction wraps.
+    const int bx = wrap(o.x0 - G::HLO - roll.x, m), by = wrap(o.y0 - G::HLO - roll.y, m);
+    const int bz = wrap(o.z0 - G::ZLO - roll.z, m);
     for (int j = tid; j < NCOMP * G::NGROUP; j += BLOCK) {
       const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
-      const int4 v = reinterpret_cast<const int4*>(s_acc)[comp * (G::PLANE / 4) + rr];
+      int4* src = reinterpret_cast<int4*>(s_acc) + comp * (G::PLANE / 4) + rr;
+      const int4 v = *src;
       if ((v.x | v.y | v.z | v.w) == 0) continue;
+      *src = make_int4(0, 0, 0, 0);
       const int q = rr % (G::SZ / 4), row = rr / (G::SZ / 4);
       const int sy = row % G::SY, sx = row / G::SY;
       float4 f;
@@ -288,129 +320,238 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
         f = make_float4(__uint2float_rn((unsigned)v.x) * is, __uint2float_rn((unsigned)v.y) * is,
                         __uint2float_rn((unsigned)v.z) * is, __uint2float_rn((unsigned)v.w) * is);
       }
-      const int gx = wrap(o.x0 - G::HLO + sx - roll.x, m), gy = wrap(o.y0 - G::HLO + sy - roll.y, m);
-      const int gz = wrap(o.z0 - G::ZLO + 4 * q - roll.z, m);
+      const int gx = wrap_up(bx + sx, m), gy = wrap_up(by + sy, m), gz = wrap_up(bz + 4 * q, m);
       float* p = mesh.p[comp] + ((size_t)gx * m + gy) * m;
       if ((gz & 3) == 0) {
         red_add_v4(p + gz, f);
       } else {  // integer part of the shift not a multiple of 4: scalar reductions, each wrapped
         atomicAdd(p + gz, f.x);
-        atomicAdd(p + wrap(gz + 1, m), f.y);
-        atomicAdd(p + wrap(gz + 2, m), f.z);
-        atomicAdd(p + wrap(gz + 3, m), f.w);
+        atomicAdd(p + wrap_up(gz + 1, m), f.y);
+        atomicAdd(p + wrap_up(gz + 2, m), f.z);
+        atomicAdd(p + wrap_up(gz + 3, m), f.w);
       }
     }
     __syncthreads();
   }
+}
+
+// ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) --------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t a = smem_u32(bar);
+  uint32_t ok = 0;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(a), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+// box (innermost first) at coordinates (c0, c1, c2) = (z, y, x); out-of-bounds elements are zero-filled
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      : "memory");
 }
 
 // ---- K4 / K7: tile gather ----------------------------------------------------------------------------
 // GRAD = false: v[i*NCOMP + a] = sum_j mesh_a[j] W_j(X_i)                                    (Eq. C.2)
 // GRAD = true : v[i*3 + b]     = sum_a coef_a(i) sum_j mesh_a[j] d/du_b W_j(X_i)             (Eq. C.6, C.12)
 // out = alpha * v (+ out if accumulate); the caller folds 1/Delta (d/dX = (1/Delta) d/du) into alpha.
-template <class T, int NCOMP, bool GRAD>
+//
+// Persistent CTAs loop over work items.  Thread 0 stages the tile + halo box of every component with one
+// TMA tensor copy each (north_star "TMA staging of mesh tiles"), completion on an mbarrier; with STAGES = 2
+// the box of the CTA's next item is in flight while the particles of the current one are interpolated.
+// TMA zero-fills what lies beyond the mesh edge, it does not wrap: tiles whose box crosses an edge (a few
+// per cent) are patched by the threads with periodic loads after the copy has landed.  roll in [0, m); when
+// roll.z is not a multiple of 4 no box start is 16-byte aligned and the threads stage everything (manual).
+template <class T, int NCOMP, bool GRAD, int STAGES>
 __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params tp, int3 roll,
+                                                  const __grid_constant__ TMapSet<NCOMP> maps,
                                                   CMeshPtrs<NCOMP> mesh, const float* __restrict__ cot,
                                                   int cstride, int ncot, float const_coef,
                                                   const float* __restrict__ wmul, float alpha,
-                                                  int accumulate, float* __restrict__ out) {
-  using G = Geo<T>;
+                                                  int accumulate, int manual, float* __restrict__ out) {
+  using G = GeoG<T>;
   constexpr int P = T::P;
-  extern __shared__ __align__(16) float s_val[];
+  constexpr int KB = 4;  // records in flight per thread
+  constexpr uint32_t BOX_BYTES = (uint32_t)(NCOMP * G::PLANE * sizeof(float));
+  extern __shared__ unsigned char s_raw[];
+  __shared__ __align__(8) uint64_t s_bar[STAGES];
+  float* s_base = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(s_raw) + 127) & ~(uintptr_t)127);
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
 
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) mbar_init(&s_bar[s], 1);
+    fence_barrier_init();
+    fence_proxy_async();
+  }
+  __syncthreads();
+
+  auto box_start = [&](const TileOrigin& o, int& cx, int& cy, int& cz) {
+    cx = wrap(o.x0 - G::HLO - roll.x, m);
+    cy = wrap(o.y0 - G::HLO - roll.y, m);
+    cz = wrap(o.z0 - G::ZLO - roll.z, m);
+  };
+  auto issue = [&](uint32_t item, int stage) {  // thread 0
+    if (manual) return;
+    const TileOrigin o = tile_origin(bv.items[item].tile, bv);
+    int cx, cy, cz;
+    box_start(o, cx, cy, cz);
+    mbar_expect_tx(&s_bar[stage], BOX_BYTES);
+#pragma unroll
+    for (int a = 0; a < NCOMP; ++a)
+      tma_load_3d(s_base + (stage * NCOMP + a) * G::PLANE_PAD, &maps.m[a], &s_bar[stage], cz, cy, cx);
+  };
+
+  uint32_t phases = 0;  // bit s: parity the next wait on stage s uses
+  int stage = 0;
+  if (tid == 0 && blockIdx.x < nitems) issue(blockIdx.x, 0);
+
   for (uint32_t it = blockIdx.x; it < nitems; it += gridDim.x) {
+    const uint32_t next = it + gridDim.x;
+    if (STAGES == 2 && tid == 0 && next < nitems) issue(next, stage ^ 1);
     const WorkItem wi = bv.items[it];
     const TileOrigin o = tile_origin(wi.tile, bv);
+    const float* s_val = s_base + stage * NCOMP * G::PLANE_PAD;
 
-    // stage tile + halo of every component
-    for (int j = tid; j < NCOMP * G::NGROUP; j += BLOCK) {
-      const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
-      const int q = rr % (G::SZ / 4), row = rr / (G::SZ / 4);
-      const int sy = row % G::SY, sx = row / G::SY;
-      const int gx = wrap(o.x0 - G::HLO + sx - roll.x, m), gy = wrap(o.y0 - G::HLO + sy - roll.y, m);
-      const int gz = wrap(o.z0 - G::ZLO + 4 * q - roll.z, m);
-      const float* p = mesh.p[comp] + ((size_t)gx * m + gy) * m;
-      float4 v;
-      if ((gz & 3) == 0) {
-        v = __ldg(reinterpret_cast<const float4*>(p + gz));
-      } else {
-        v = make_float4(__ldg(p + gz), __ldg(p + wrap(gz + 1, m)), __ldg(p + wrap(gz + 2, m)),
-                        __ldg(p + wrap(gz + 3, m)));
-      }
-      reinterpret_cast<float4*>(s_val)[comp * (G::PLANE / 4) + rr] = v;
+    // first batch of records: in flight while the box lands
+    uint4 r[KB];
+#pragma unroll
+    for (int k = 0; k < KB; ++k) {
+      const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
+      if (i < wi.end) r[k] = bv.rec[i];
     }
-    __syncthreads();
 
-    for (uint32_t i = wi.begin + tid; i < wi.end; i += BLOCK) {
-      const uint4 r = bv.rec[i];
-      int sx, sy, sz;
-      float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
-      T::template axis<GRAD>(apply_shift(r.x, tp.frac[0]), tp, sx, wx, dx);
-      T::template axis<GRAD>(apply_shift(r.y, tp.frac[1]), tp, sy, wy, dy);
-      T::template axis<GRAD>(apply_shift(r.z, tp.frac[2]), tp, sz, wz, dz);
-      sz += G::ZLO - G::HLO;
-      const int base = (sx * G::SY + sy) * G::SZ + sz;
-      if (!GRAD) {
-        float acc[NCOMP];
+    if (!manual) {
+      mbar_wait(&s_bar[stage], (phases >> stage) & 1u);
+      phases ^= 1u << stage;
+    }
+
+    int cx, cy, cz;
+    box_start(o, cx, cy, cz);
+    if (manual || cx + G::SX > m || cy + G::SY > m || cz + G::SZ > m) {  // uniform: box crosses a mesh edge
+      float* s_w = s_base + stage * NCOMP * G::PLANE_PAD;
+      for (int j = tid; j < NCOMP * G::NGROUP; j += BLOCK) {
+        const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
+        const int q = rr % (G::SZ / 4), row = rr / (G::SZ / 4);
+        const int sy = row % G::SY, sx = row / G::SY;
+        if (!manual && cx + sx < m && cy + sy < m && cz + 4 * q + 3 < m) continue;  // TMA delivered it
+        const float* p = mesh.p[comp] + ((size_t)wrap_up(cx + sx, m) * m + wrap_up(cy + sy, m)) * m;
+        const int gz = cz + 4 * q;
+        const float4 v = make_float4(__ldg(p + wrap_up(gz, m)), __ldg(p + wrap_up(gz + 1, m)),
+                                     __ldg(p + wrap_up(gz + 2, m)), __ldg(p + wrap_up(gz + 3, m)));
+        reinterpret_cast<float4*>(s_w + comp * G::PLANE_PAD)[rr] = v;
+      }
+      fence_proxy_async();  // generic-proxy writes before the async proxy refills this buffer
+      __syncthreads();
+    }
+
+    for (uint32_t b0 = wi.begin; b0 < wi.end; b0 += KB * BLOCK) {
+      if (b0 != wi.begin) {
 #pragma unroll
-        for (int a = 0; a < NCOMP; ++a) acc[a] = 0.0f;
-#pragma unroll
-        for (int a = 0; a < P; ++a)
-#pragma unroll
-          for (int b = 0; b < P; ++b) {
-            const float wxy = wx[a] * wy[b];
-            const int row = base + (a * G::SY + b) * G::SZ;
-#pragma unroll
-            for (int c = 0; c < P; ++c) {
-              const float wxyz = wxy * wz[c];
-#pragma unroll
-              for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, s_val[q * G::PLANE + row + c], acc[q]);
-            }
-          }
-#pragma unroll
-        for (int a = 0; a < NCOMP; ++a) {
-          float* dst = out + (size_t)r.w * NCOMP + a;
-          *dst = accumulate ? fmaf(alpha, acc[a], *dst) : alpha * acc[a];
+        for (int k = 0; k < KB; ++k) {
+          const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
+          if (i < wi.end) r[k] = bv.rec[i];
         }
-      } else {
-        float coef[NCOMP];
-        const float cc = const_coef * (wmul ? __ldg(wmul + r.w) : 1.0f);
+      }
 #pragma unroll
-        for (int a = 0; a < NCOMP; ++a) coef[a] = a < ncot ? __ldg(cot + (size_t)r.w * cstride + a) : cc;
-        float gx = 0.0f, gy = 0.0f, gz = 0.0f;
+      for (int k = 0; k < KB; ++k) {
+        const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
+        if (i >= wi.end) continue;
+        const uint4 rk = r[k];
+        int sx, sy, sz;
+        float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
+        T::template axis<GRAD>(apply_shift(rk.x, tp.frac[0]), tp, sx, wx, dx);
+        T::template axis<GRAD>(apply_shift(rk.y, tp.frac[1]), tp, sy, wy, dy);
+        T::template axis<GRAD>(apply_shift(rk.z, tp.frac[2]), tp, sz, wz, dz);
+        sz += G::ZLO - G::HLO;
+        const int base = (sx * G::SY + sy) * G::SZ + sz;
+        if (!GRAD) {
+          float acc[NCOMP];
 #pragma unroll
-        for (int a = 0; a < P; ++a)
+          for (int a = 0; a < NCOMP; ++a) acc[a] = 0.0f;
 #pragma unroll
-          for (int b = 0; b < P; ++b) {
-            const int row = base + (a * G::SY + b) * G::SZ;
-            const float wdx = dx[a] * wy[b], wdy = wx[a] * dy[b], wxy = wx[a] * wy[b];
+          for (int a = 0; a < P; ++a)
 #pragma unroll
-            for (int c = 0; c < P; ++c) {
-              float val = 0.0f;
+            for (int b = 0; b < P; ++b) {
+              const float wxy = wx[a] * wy[b];
+              const int row = base + (a * G::SY + b) * G::SZ;
 #pragma unroll
-              for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], s_val[q * G::PLANE + row + c], val);
-              gx = fmaf(wdx * wz[c], val, gx);
-              gy = fmaf(wdy * wz[c], val, gy);
-              gz = fmaf(wxy * dz[c], val, gz);
+              for (int c = 0; c < P; ++c) {
+                const float wxyz = wxy * wz[c];
+#pragma unroll
+                for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, s_val[q * G::PLANE_PAD + row + c], acc[q]);
+              }
             }
+#pragma unroll
+          for (int a = 0; a < NCOMP; ++a) {
+            float* dst = out + (size_t)rk.w * NCOMP + a;
+            *dst = accumulate ? fmaf(alpha, acc[a], *dst) : alpha * acc[a];
           }
-        float* dst = out + (size_t)r.w * 3;
-        dst[0] = accumulate ? fmaf(alpha, gx, dst[0]) : alpha * gx;
-        dst[1] = accumulate ? fmaf(alpha, gy, dst[1]) : alpha * gy;
-        dst[2] = accumulate ? fmaf(alpha, gz, dst[2]) : alpha * gz;
+        } else {
+          float coef[NCOMP];
+          const float cc = const_coef * (wmul ? __ldg(wmul + rk.w) : 1.0f);
+#pragma unroll
+          for (int a = 0; a < NCOMP; ++a) coef[a] = a < ncot ? __ldg(cot + (size_t)rk.w * cstride + a) : cc;
+          float gx = 0.0f, gy = 0.0f, gz = 0.0f;
+#pragma unroll
+          for (int a = 0; a < P; ++a)
+#pragma unroll
+            for (int b = 0; b < P; ++b) {
+              const int row = base + (a * G::SY + b) * G::SZ;
+              const float wdx = dx[a] * wy[b], wdy = wx[a] * dy[b], wxy = wx[a] * wy[b];
+#pragma unroll
+              for (int c = 0; c < P; ++c) {
+                float val = 0.0f;
+#pragma unroll
+                for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], s_val[q * G::PLANE_PAD + row + c], val);
+                gx = fmaf(wdx * wz[c], val, gx);
+                gy = fmaf(wdy * wz[c], val, gy);
+                gz = fmaf(wxy * dz[c], val, gz);
+              }
+            }
+          float* dst = out + (size_t)rk.w * 3;
+          dst[0] = accumulate ? fmaf(alpha, gx, dst[0]) : alpha * gx;
+          dst[1] = accumulate ? fmaf(alpha, gy, dst[1]) : alpha * gy;
+          dst[2] = accumulate ? fmaf(alpha, gz, dst[2]) : alpha * gz;
+        }
       }
     }
-    __syncthreads();
+    __syncthreads();  // every thread is done with this stage: it may be refilled
+    if (STAGES == 2) {
+      stage ^= 1;
+    } else if (tid == 0 && next < nitems) {
+      issue(next, 0);
+    }
   }
 }
 
 // ---- host-side launch helpers ------------------------------------------------------------------------
-inline int mesh_grid(const Ctx* c) {
+inline int norm_roll(int r, int m) {
+  r %= m;
+  return r < 0 ? r + m : r;
+}
+
+// Grid of a persistent mesh kernel: resident CTAs per SM x SMs, capped by an upper bound of the item count.
+inline int mesh_grid(const Ctx* c, int occ) {
   int64_t bound = (int64_t)c->ntiles + c->bin_n / CHUNK + 1;
-  int64_t cap = (int64_t)c->num_sms * 8;
+  int64_t cap = (int64_t)c->num_sms * (occ < 1 ? 1 : occ);
   return (int)(bound < cap ? bound : cap);
 }
 
@@ -420,14 +561,18 @@ int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const f
   using G = Geo<T>;
   const size_t smem = sizeof(int) * (size_t)NCOMP * G::PLANE;
   auto kern = k_scatter<T, NCOMP, WEIGHTED>;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static int occ = 0;
+  if (!occ) {
     PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_done = true;
+    PM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLOCK, smem));
+    if (occ < 1) return fail(c, PM_ECUDA, "scatter kernel does not fit on an SM");
   }
   MeshPtrs<NCOMP> mp;
   for (int a = 0; a < NCOMP; ++a) mp.p[a] = mesh[a];
-  kern<<<mesh_grid(c), BLOCK, smem, st>>>(bin_view(c), tp, make_int3(roll[0], roll[1], roll[2]), wsrc, wstride, mp);
+  const int m = c->mg;
+  kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp,
+                                               make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m)),
+                                               wsrc, wstride, mp);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;
@@ -437,19 +582,28 @@ template <class T, int NCOMP, bool GRAD>
 int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const float* const mesh[],
                const float* cot, int cstride, int ncot, float const_coef, const float* wmul, float alpha,
                bool accumulate, float* out, cudaStream_t st) {
-  using G = Geo<T>;
-  const size_t smem = sizeof(float) * (size_t)NCOMP * G::PLANE;
-  auto kern = k_gather<T, NCOMP, GRAD>;
-  static bool attr_done = false;
-  if (!attr_done) {
+  using G = GeoG<T>;
+  constexpr size_t stage_bytes = sizeof(float) * (size_t)NCOMP * G::PLANE_PAD;
+  constexpr int STAGES = 2 * stage_bytes <= 100 * 1024 ? 2 : 1;
+  constexpr size_t smem = STAGES * stage_bytes + 128;
+  auto kern = k_gather<T, NCOMP, GRAD, STAGES>;
+  static int occ = 0;
+  if (!occ) {
     PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_done = true;
+    PM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLOCK, smem));
+    if (occ < 1) return fail(c, PM_ECUDA, "gather kernel does not fit on an SM");
   }
   CMeshPtrs<NCOMP> mp;
-  for (int a = 0; a < NCOMP; ++a) mp.p[a] = mesh[a];
+  TMapSet<NCOMP> maps;
+  const int m = c->mg;
+  for (int a = 0; a < NCOMP; ++a) {
+    mp.p[a] = mesh[a];
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::SZ, &maps.m[a]));
+  }
   const float a_eff = GRAD ? (float)((double)alpha * (double)c->mg / c->p.box) : alpha;
-  kern<<<mesh_grid(c), BLOCK, smem, st>>>(bin_view(c), tp, make_int3(roll[0], roll[1], roll[2]), mp, cot, cstride,
-                                          ncot, const_coef, wmul, a_eff, accumulate ? 1 : 0, out);
+  const int3 nr = make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m));
+  kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp, nr, maps, mp, cot, cstride, ncot, const_coef, wmul,
+                                               a_eff, accumulate ? 1 : 0, (nr.z & 3) ? 1 : 0, out);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

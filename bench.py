@@ -107,6 +107,27 @@ def oracle_sample_run(cfg_name: str, n_p: int):
     return time.perf_counter() - t0, pos.shape[0]
 
 
+def replica_seed(seed: int, rank: int) -> int:
+    """Seed of rank's independent replica (replicas only, no data-path collective)."""
+    return int(seed) + 100 * int(rank)
+
+
+def max_over_ranks(values, world: int, device="cpu"):
+    """Element-wise MAX of per-rank timings over all ranks (the only collective of the bench)."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_rate(world: int, units_per_rank: int, steps: int, ms_total: float) -> float:
+    """Units all ranks processed / the slowest rank's time (weak scaling: per-rank work is fixed)."""
+    return world * units_per_rank * steps / (ms_total * 1e-3)
+
+
 def host_threads() -> int:
     try:
         return len(os.sched_getaffinity(0))
@@ -166,7 +187,7 @@ def run_ours(args) -> int:
     if args.n_p:
         pos_np, c = gen.make_config_positions(args.config, n_p=args.n_p)
     else:
-        c["seed"] = c["seed"] + 100 * rank
+        c["seed"] = replica_seed(c["seed"], rank)
         if c.get("clustered"):
             pos_np = gen.clustered_halos(c["n_p"] ** 3, c["m"], c["box"], c["seed"],
                                          lattice_shape=(c["n_p"], c["n_p"], c["n_p"] // 2), rms_cells=c["rms"])
@@ -228,17 +249,14 @@ def run_ours(args) -> int:
     e2e_s = time.perf_counter() - t0
     checksum = float(force_host[:: max(1, n // 1000)].double().abs().sum())
 
-    t = torch.tensor([ms_total, e2e_s * 1e3], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, e2e_ms = float(t[0]), float(t[1])
+    ms_total, e2e_ms = max_over_ranks([ms_total, e2e_s * 1e3], world, device="cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
 
-    value = world * n * args.steps / (ms_total * 1e-3)
-    e2e_value = world * n * e2e_steps / (e2e_ms * 1e-3)
+    value = whole_job_rate(world, n, args.steps, ms_total)
+    e2e_value = whole_job_rate(world, n, e2e_steps, e2e_ms)
 
     # ---- roofline of the dominant hand-written kernel -----------------------------------------------------
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")

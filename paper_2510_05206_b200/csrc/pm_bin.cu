@@ -1,7 +1,8 @@
 // pm_bin.cu -- a0: on-device counting sort of particles into mesh tiles (north_star: "Particles are
 // sorted into cell tiles with an on-device counting/Morton sort").  Not in the paper; the build's own step.
 //
-//   pass 1  k_count   : cell coordinate in fp64 from the fp32 position, tile histogram (warp-aggregated)
+//   pass 1  k_count   : cell coordinate (fp64-accurate, see cell_coord) from the fp32 position, tile histogram
+//                       (warp-aggregated)
 //   scan    k_scan_*  : exclusive scans of the tile counts and of the per-tile work-item counts
 //   pass 2  k_permute : recompute the coordinate, claim a slot (warp-aggregated, order-preserving inside a
 //                       warp), store the record {ux, uy, uz, i} with tile-local fixed-point coordinates
@@ -14,35 +15,57 @@ namespace pmf {
 
 struct BinGeom {
   int m, ntx, nty, ntz, xbl;
-  double inv_dx;  // m / box
+  float c_hi, c_lo;  // m / box split into two floats (c_hi + c_lo = m/box to ~2^-48)
+  double inv_dx;     // m / box
 };
 
-// u = x * m/L in fp64, wrapped into [0, m).  (SURVEY 7 "hard parts": the fp32 product is not enough.)
-__device__ __forceinline__ double cell_coord(float x, const BinGeom& g) {
-  double u = (double)x * g.inv_dx;
-  const double dm = (double)g.m;
-  if (u < 0.0 || u >= dm) {
+// Cell coordinate u = x * m/L of one axis as (integer cell in [0, m), 26-bit fraction).
+// SURVEY 7 "hard parts": the plain fp32 product is not accurate enough.  Fast path: error-free fp32 product
+// p + e = x * (c_hi + c_lo) (FMA residual), p split into round(p) and an exact remainder -- fp32 pipes only, one
+// float->int conversion.  Anything outside [0, m) (x outside [0, L), or rounded up to m) takes the fp64 path.
+// Both binning passes call this same function, so they always agree on the tile of a particle.
+__device__ __forceinline__ void cell_coord(float x, const BinGeom& g, int& cell, uint32_t& frac) {
+  const float p = __fmul_rn(x, g.c_hi);
+  const float e = __fmaf_rn(x, g.c_lo, __fmaf_rn(x, g.c_hi, -p));
+  const float t = __fadd_rn(p, 12582912.0f);  // 1.5 * 2^23: the integer nearest to p sits in the low mantissa bits
+  const float r = __fsub_rn(p, __fsub_rn(t, 12582912.0f));  // exact, in [-1/2, 1/2]
+  const int fi = __float2int_rn(__fadd_rn(r, e) * (float)REC_ONE);
+  cell = (__float_as_int(t) - 0x4B400000) + (fi >> REC_FRAC);
+  frac = (uint32_t)fi & REC_MASK;
+  if (!(fabsf(p) < 4.0e6f) || (unsigned)cell >= (unsigned)g.m) {  // rare: wrap in fp64
+    double u = (double)x * g.inv_dx;
+    const double dm = (double)g.m;
     u -= dm * floor(u / dm);
-    if (!(u >= 0.0) || u >= dm) u = 0.0;
+    if (!(u >= 0.0) || u >= dm) u = 0.0;  // non-finite input, or rounded up to m
+    const double fl = floor(u);
+    cell = (int)fl;
+    uint32_t f = (uint32_t)__double2ll_rn((u - fl) * (double)REC_ONE);
+    if (f >= REC_ONE) f = REC_ONE - 1u;
+    frac = f;
   }
-  return u;
 }
 
 __device__ __forceinline__ uint32_t tile_and_local(float x, float y, float z, const BinGeom& g, uint32_t& fx,
                                                    uint32_t& fy, uint32_t& fz) {
-  const double ux = cell_coord(x, g), uy = cell_coord(y, g), uz = cell_coord(z, g);
-  const int tx = (int)ux / TX, ty = (int)uy / TY, tz = (int)uz / TZ;
-  const double s = (double)REC_ONE;
-  // (u_local + REC_BIAS) * 2^REC_FRAC, clamped below the next tile so the integer part stays in-tile
-  fx = min((uint32_t)__double2ll_rn((ux - tx * TX + REC_BIAS) * s), (uint32_t)((TX + REC_BIAS) * REC_ONE - 1u));
-  fy = min((uint32_t)__double2ll_rn((uy - ty * TY + REC_BIAS) * s), (uint32_t)((TY + REC_BIAS) * REC_ONE - 1u));
-  fz = min((uint32_t)__double2ll_rn((uz - tz * TZ + REC_BIAS) * s), (uint32_t)((TZ + REC_BIAS) * REC_ONE - 1u));
+  int cx, cy, cz;
+  cell_coord(x, g, cx, fx);
+  cell_coord(y, g, cy, fy);
+  cell_coord(z, g, cz, fz);
+  const int tx = cx / TX, ty = cy / TY, tz = cz / TZ;
+  // (u_local + REC_BIAS) * 2^REC_FRAC
+  fx |= (uint32_t)(cx - tx * TX + REC_BIAS) << REC_FRAC;
+  fy |= (uint32_t)(cy - ty * TY + REC_BIAS) << REC_FRAC;
+  fz |= (uint32_t)(cz - tz * TZ + REC_BIAS) << REC_FRAC;
   return tile_id(tx, ty, tz, g.nty, g.ntz, g.xbl);
 }
 
 __device__ __forceinline__ uint32_t tile_only(float x, float y, float z, const BinGeom& g) {
-  const int tx = (int)cell_coord(x, g) / TX, ty = (int)cell_coord(y, g) / TY, tz = (int)cell_coord(z, g) / TZ;
-  return tile_id(tx, ty, tz, g.nty, g.ntz, g.xbl);
+  int cx, cy, cz;
+  uint32_t f;
+  cell_coord(x, g, cx, f);
+  cell_coord(y, g, cy, f);
+  cell_coord(z, g, cz, f);
+  return tile_id(cx / TX, cy / TY, cz / TZ, g.nty, g.ntz, g.xbl);
 }
 
 // The lanes of a warp hold 32 CONSECUTIVE particles.  Each run of equal keys elects its first lane, which
@@ -213,18 +236,25 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_final(uint32_t* __restrict__ cn
 }
 
 __global__ void __launch_bounds__(256) k_items(const uint32_t* __restrict__ tile_off,
-                                               const uint32_t* __restrict__ item_off, int ntiles,
-                                               WorkItem* __restrict__ items) {
+                                               const uint32_t* __restrict__ item_off, int ntiles, int nty, int ntz,
+                                               int xbl, WorkItem* __restrict__ items) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= ntiles) return;
   const uint32_t b = tile_off[t], e = tile_off[t + 1];
   uint32_t it = item_off[t];
+  // inverse of tile_id()
+  const int tz = t % ntz;
+  int r = t / ntz;
+  const int xl = r & ((1 << xbl) - 1);
+  r >>= xbl;
+  const int ty = r % nty, tx = ((r / nty) << xbl) | xl;
+  const uint32_t txyz = (uint32_t)tx | ((uint32_t)ty << 10) | ((uint32_t)tz << 20);
   for (uint32_t s = b; s < e; s += CHUNK) {
     WorkItem w;
     w.tile = (uint32_t)t;
     w.begin = s;
     w.end = min(s + (uint32_t)CHUNK, e);
-    w.pad = 0;
+    w.txyz = txyz;
     items[it++] = w;
   }
 }
@@ -234,6 +264,7 @@ BinView bin_view(const Ctx* c) {
   v.rec = c->rec;
   v.items = c->items;
   v.nitems = c->nitems;
+  v.sched = c->sched;
   v.m = c->mg;
   v.ntx = c->ntx;
   v.nty = c->nty;
@@ -254,6 +285,8 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   g.ntz = c->ntz;
   g.xbl = c->xbl;
   g.inv_dx = (double)c->mg / c->p.box;
+  g.c_hi = (float)g.inv_dx;
+  g.c_lo = (float)(g.inv_dx - (double)g.c_hi);
   const int nt = c->ntiles;
   const int nb = (nt + SCAN_B - 1) / SCAN_B;
   uint2* partial = reinterpret_cast<uint2*>(c->scan_tmp);
@@ -270,7 +303,7 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   k_scan_partials<<<1, SCAN_T, 0, st>>>(partial, nb, c->tile_off, c->item_off, nt, c->nitems);
   k_scan_final<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, c->tile_off, c->item_off);
   if (N > 0) k_bin_pass<true><<<grid, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, c->tile_off, c->rec, aligned);
-  k_items<<<(nt + 255) / 256, 256, 0, st>>>(c->tile_off, c->item_off, nt, c->items);
+  k_items<<<(nt + 255) / 256, 256, 0, st>>>(c->tile_off, c->item_off, nt, c->nty, c->ntz, c->xbl, c->items);
   count_launch(c, N > 0 ? 6 : 4);
   PM_CUDA(c, cudaGetLastError());
   c->bin_valid = true;

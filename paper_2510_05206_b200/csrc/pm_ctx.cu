@@ -65,7 +65,7 @@ int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMa
   const cuuint32_t estr[3] = {1, 1, 1};
   const CUresult r = g_encode_tiled(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides,
                                     box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                    (getenv("PMF_TMA_PROMO") ? (CUtensorMapL2promotion)atoi(getenv("PMF_TMA_PROMO")) : CU_TENSOR_MAP_L2_PROMOTION_L2_128B), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(c, PM_ECUDA, "cuTensorMapEncodeTiled failed: CUresult %d (box %d x %d x %d)", (int)r, sx, sy, sz);
   return PM_OK;
 }
@@ -253,6 +253,8 @@ static int build(Ctx* c) {
   PM_CUDA(c, cudaMalloc((void**)&c->items, sizeof(WorkItem) * (size_t)c->max_items));
   PM_CUDA(c, cudaMalloc((void**)&c->nitems, sizeof(uint32_t)));
   PM_CUDA(c, cudaMemset(c->nitems, 0, sizeof(uint32_t)));
+  PM_CUDA(c, cudaMalloc((void**)&c->sched, 2 * sizeof(uint32_t)));
+  PM_CUDA(c, cudaMemset(c->sched, 0, 2 * sizeof(uint32_t)));
 
   // cuFFT plans (library call, reported as its own line; north_star "may call cuFFT")
   size_t ws1 = 0, ws2 = 0;
@@ -294,7 +296,7 @@ static void teardown(Ctx* c) {
     cufftDestroy(c->plan_c2r);
   }
   void* ptrs[] = {c->tab_grad, c->tab_lap, c->tab_win, c->tab_cos, c->tab_sin, c->rec, c->tile_cnt,
-                  c->tile_off, c->item_off, c->scan_tmp, c->items, c->nitems, c->fft_work, c->rho[0],
+                  c->tile_off, c->item_off, c->scan_tmp, c->items, c->nitems, c->sched, c->fft_work, c->rho[0],
                   c->rho[1], c->dhat[0], c->dhat[1], c->ghat[0], c->ghat[1], c->ghat[2], c->g[0],
                   c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->host_pos_dev,
                   c->host_force_dev};

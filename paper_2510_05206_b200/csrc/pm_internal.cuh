@@ -20,7 +20,8 @@
 namespace pmf {
 
 // ---- tile geometry ------------------------------------------------------------------------------
-constexpr int TX = 8, TY = 8, TZ = 16;  // cells per tile
+constexpr int TX = 8, TY = 8, TZ = 32;  // cells per tile: a warp's 32 consecutive (Lagrangian-order) records fill
+                                        // one z row, so their shared-memory accesses fall in 32 different banks
 constexpr int BLOCK = 256;              // threads per CTA of the scatter / gather kernels
 constexpr int PPT = 8;                  // particles per thread and work item
 constexpr int CHUNK = BLOCK * PPT;      // max particles per work item
@@ -30,7 +31,8 @@ constexpr uint32_t REC_ONE = 1u << REC_FRAC;
 constexpr uint32_t REC_MASK = REC_ONE - 1u;
 
 struct WorkItem {
-  uint32_t tile, begin, end, pad;
+  uint32_t tile, begin, end;
+  uint32_t txyz;  // tile coordinates packed tx | ty << 10 | tz << 20 (written by k_items: no division in the hot kernels)
 };
 
 // Everything a scatter / gather kernel needs to know about the grid and the binned particles.
@@ -38,6 +40,7 @@ struct BinView {
   const uint4* rec;
   const WorkItem* items;
   const uint32_t* nitems;
+  uint32_t* sched;  // [2]: next-item counter and finished-CTA counter of the dynamic tile schedule (zero between launches)
   int m, ntx, nty, ntz;
   int xbl;  // log2 of xb; tiles are numbered ((tx / xb * nty + ty) * xb + tx % xb) * ntz + tz, see tile_id()
 };
@@ -107,6 +110,7 @@ struct Ctx {
   uint32_t* scan_tmp;   // [2 * nblocks_scan + 2]
   WorkItem* items;      // [max_items]
   uint32_t* nitems;     // device scalar
+  uint32_t* sched;      // [2] dynamic-schedule counters, see BinView
   int64_t max_items;
   const float* bin_pos; // pointer the records were built from
   int64_t bin_n;

@@ -19,42 +19,71 @@ struct KTabs {
 };
 
 constexpr int KS_BLOCK = 128;
+constexpr int KS_ROWS = 4;  // (ix, iy .. iy+3) rows per CTA: 4 independent loads in flight per thread, one table read
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
   return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
 
-// One CTA per (ix, iy) row of the half-complex grid; threads run along iz.
+// per-row (ix, iy) factors of the multiplier
+struct RowFac {
+  double lxy, wxy, dxv, dyv;
+  float2 pxy;
+};
+__device__ __forceinline__ RowFac row_factors(const KTabs& t, int ix, int iy, bool phase, float sgn) {
+  RowFac r;
+  r.lxy = t.lap[ix] + t.lap[iy];
+  r.wxy = t.win[ix] * t.win[iy];
+  r.dxv = t.grad[ix];
+  r.dyv = t.grad[iy];
+  r.pxy = make_float2(1.f, 0.f);
+  if (phase) {
+    const double cr = t.pc[ix] * t.pc[iy] - t.ps[ix] * t.ps[iy];
+    const double ci = t.pc[ix] * t.ps[iy] + t.ps[ix] * t.pc[iy];
+    r.pxy = make_float2((float)cr, sgn * (float)ci);
+  }
+  return r;
+}
+
+// One CTA per KS_ROWS consecutive (ix, iy) rows of the half-complex grid (m is a multiple of 4, so the rows of
+// a CTA share ix); threads run along iz.
 __global__ void __launch_bounds__(KS_BLOCK) k_kspace_fwd(KTabs t, const float2* __restrict__ d1,
                                                          const float2* __restrict__ d2,
                                                          float2* __restrict__ g0, float2* __restrict__ g1,
                                                          float2* __restrict__ g2, double coeff_eff) {
-  const int row = blockIdx.x;
-  const int ix = row / t.m, iy = row - ix * t.m;
-  const double lxy = t.lap[ix] + t.lap[iy];
-  const double wxy = t.win[ix] * t.win[iy];
-  const double dxv = t.grad[ix], dyv = t.grad[iy];
-  float2 pxy = make_float2(1.f, 0.f);
-  if (d2) {
-    const double cr = t.pc[ix] * t.pc[iy] - t.ps[ix] * t.ps[iy];
-    const double ci = t.pc[ix] * t.ps[iy] + t.ps[ix] * t.pc[iy];
-    pxy = make_float2((float)cr, (float)ci);
-  }
-  const size_t base = (size_t)row * t.hz;
+  const int row0 = blockIdx.x * KS_ROWS;
+  const int ix = row0 / t.m, iy0 = row0 - ix * t.m;
+  RowFac rf[KS_ROWS];
+#pragma unroll
+  for (int r = 0; r < KS_ROWS; ++r) rf[r] = row_factors(t, ix, iy0 + r, d2 != nullptr, 1.f);
+  const size_t base = (size_t)row0 * t.hz;
   for (int iz = threadIdx.x; iz < t.hz; iz += KS_BLOCK) {
-    const double den = (lxy + t.lap[iz]) * (wxy * t.win[iz]);
-    const double green = (den != 0.0) ? coeff_eff / den : 0.0;  // n = 0 and dropped modes -> 0
-    float2 d = d1[base + iz];
+    float2 d[KS_ROWS], e[KS_ROWS];
+#pragma unroll
+    for (int r = 0; r < KS_ROWS; ++r) d[r] = __ldcs(d1 + base + (size_t)r * t.hz + iz);
     if (d2) {
-      const float2 pz = make_float2((float)t.pc[iz], (float)t.ps[iz]);
-      const float2 e = cmul(cmul(pxy, pz), d2[base + iz]);
-      d = make_float2(0.5f * (d.x + e.x), 0.5f * (d.y + e.y));
+#pragma unroll
+      for (int r = 0; r < KS_ROWS; ++r) e[r] = __ldcs(d2 + base + (size_t)r * t.hz + iz);
     }
-    // -i D green (re + i im) = D green (im - i re)
-    const float mx = (float)(dxv * green), my = (float)(dyv * green), mz = (float)(t.grad[iz] * green);
-    g0[base + iz] = make_float2(mx * d.y, -mx * d.x);
-    g1[base + iz] = make_float2(my * d.y, -my * d.x);
-    g2[base + iz] = make_float2(mz * d.y, -mz * d.x);
+    const double lz = t.lap[iz], wz = t.win[iz], gz = t.grad[iz];
+    float2 pz = make_float2(1.f, 0.f);
+    if (d2) pz = make_float2((float)t.pc[iz], (float)t.ps[iz]);
+#pragma unroll
+    for (int r = 0; r < KS_ROWS; ++r) {
+      const double den = (rf[r].lxy + lz) * (rf[r].wxy * wz);
+      const double green = (den != 0.0) ? coeff_eff / den : 0.0;  // n = 0 and dropped modes -> 0
+      float2 v = d[r];
+      if (d2) {
+        const float2 q = cmul(cmul(rf[r].pxy, pz), e[r]);
+        v = make_float2(0.5f * (v.x + q.x), 0.5f * (v.y + q.y));
+      }
+      // -i D green (re + i im) = D green (im - i re)
+      const float mx = (float)(rf[r].dxv * green), my = (float)(rf[r].dyv * green), mz = (float)(gz * green);
+      const size_t o = base + (size_t)r * t.hz + iz;
+      g0[o] = make_float2(mx * v.y, -mx * v.x);
+      g1[o] = make_float2(my * v.y, -my * v.x);
+      g2[o] = make_float2(mz * v.y, -mz * v.x);
+    }
   }
 }
 
@@ -62,32 +91,39 @@ __global__ void __launch_bounds__(KS_BLOCK) k_kspace_tr(KTabs t, const float2* _
                                                         const float2* __restrict__ g1,
                                                         const float2* __restrict__ g2, float2* __restrict__ q1,
                                                         float2* __restrict__ q2, double coeff_eff) {
-  const int row = blockIdx.x;
-  const int ix = row / t.m, iy = row - ix * t.m;
-  const double lxy = t.lap[ix] + t.lap[iy];
-  const double wxy = t.win[ix] * t.win[iy];
-  const double dxv = t.grad[ix], dyv = t.grad[iy];
-  float2 pxy = make_float2(1.f, 0.f);
-  if (q2) {  // conj of the interlace phase
-    const double cr = t.pc[ix] * t.pc[iy] - t.ps[ix] * t.ps[iy];
-    const double ci = t.pc[ix] * t.ps[iy] + t.ps[ix] * t.pc[iy];
-    pxy = make_float2((float)cr, (float)-ci);
-  }
-  const size_t base = (size_t)row * t.hz;
+  const int row0 = blockIdx.x * KS_ROWS;
+  const int ix = row0 / t.m, iy0 = row0 - ix * t.m;
+  RowFac rf[KS_ROWS];
+#pragma unroll
+  for (int r = 0; r < KS_ROWS; ++r) rf[r] = row_factors(t, ix, iy0 + r, q2 != nullptr, -1.f);  // conj of the phase
+  const size_t base = (size_t)row0 * t.hz;
   for (int iz = threadIdx.x; iz < t.hz; iz += KS_BLOCK) {
-    const double den = (lxy + t.lap[iz]) * (wxy * t.win[iz]);
-    const double green = (den != 0.0) ? coeff_eff / den : 0.0;
-    const float mx = (float)(dxv * green), my = (float)(dyv * green), mz = (float)(t.grad[iz] * green);
-    const float2 a = g0[base + iz], b = g1[base + iz], c = g2[base + iz];
-    // conj(S_a) = +i D_a green:  q = i * sum_a m_a (re_a + i im_a)
-    float2 q = make_float2(-(mx * a.y + my * b.y + mz * c.y), mx * a.x + my * b.x + mz * c.x);
-    if (q2) {
-      q.x *= 0.5f;
-      q.y *= 0.5f;
-      const float2 pz = make_float2((float)t.pc[iz], (float)-t.ps[iz]);
-      q2[base + iz] = cmul(cmul(pxy, pz), q);
+    float2 a[KS_ROWS], b[KS_ROWS], c[KS_ROWS];
+#pragma unroll
+    for (int r = 0; r < KS_ROWS; ++r) {
+      const size_t o = base + (size_t)r * t.hz + iz;
+      a[r] = __ldcs(g0 + o);
+      b[r] = __ldcs(g1 + o);
+      c[r] = __ldcs(g2 + o);
     }
-    q1[base + iz] = q;
+    const double lz = t.lap[iz], wz = t.win[iz], gz = t.grad[iz];
+    float2 pz = make_float2(1.f, 0.f);
+    if (q2) pz = make_float2((float)t.pc[iz], (float)-t.ps[iz]);
+#pragma unroll
+    for (int r = 0; r < KS_ROWS; ++r) {
+      const double den = (rf[r].lxy + lz) * (rf[r].wxy * wz);
+      const double green = (den != 0.0) ? coeff_eff / den : 0.0;
+      const float mx = (float)(rf[r].dxv * green), my = (float)(rf[r].dyv * green), mz = (float)(gz * green);
+      // conj(S_a) = +i D_a green:  q = i * sum_a m_a (re_a + i im_a)
+      float2 q = make_float2(-(mx * a[r].y + my * b[r].y + mz * c[r].y), mx * a[r].x + my * b[r].x + mz * c[r].x);
+      const size_t o = base + (size_t)r * t.hz + iz;
+      if (q2) {
+        q.x *= 0.5f;
+        q.y *= 0.5f;
+        q2[o] = cmul(cmul(rf[r].pxy, pz), q);
+      }
+      q1[o] = q;
+    }
   }
 }
 
@@ -105,7 +141,7 @@ static KTabs tabs_of(const Ctx* c) {
 
 int launch_kspace_forward(Ctx* c, const float2* d1, const float2* d2, float2* const ghat[3], double coeff_eff,
                           cudaStream_t st) {
-  k_kspace_fwd<<<c->mg * c->mg, KS_BLOCK, 0, st>>>(tabs_of(c), d1, d2, ghat[0], ghat[1], ghat[2], coeff_eff);
+  k_kspace_fwd<<<c->mg * c->mg / KS_ROWS, KS_BLOCK, 0, st>>>(tabs_of(c), d1, d2, ghat[0], ghat[1], ghat[2], coeff_eff);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;
@@ -113,7 +149,7 @@ int launch_kspace_forward(Ctx* c, const float2* d1, const float2* d2, float2* co
 
 int launch_kspace_transpose(Ctx* c, const float2* const gh[3], float2* q1, float2* q2, double coeff_eff,
                             cudaStream_t st) {
-  k_kspace_tr<<<c->mg * c->mg, KS_BLOCK, 0, st>>>(tabs_of(c), gh[0], gh[1], gh[2], q1, q2, coeff_eff);
+  k_kspace_tr<<<c->mg * c->mg / KS_ROWS, KS_BLOCK, 0, st>>>(tabs_of(c), gh[0], gh[1], gh[2], q1, q2, coeff_eff);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

@@ -10,6 +10,7 @@
 //            P^3 nodes from there.
 #pragma once
 #include <cuda.h>
+#include <stdlib.h>
 
 #include "pm_internal.cuh"
 
@@ -22,6 +23,7 @@ namespace pmf {
 template <int ORDER, bool SHIFTED>
 struct PMTraits {
   static constexpr int P = ORDER;
+  static constexpr bool SHIFT = SHIFTED;  // a fractional grid shift is subtracted from the record coordinate
   static constexpr int HLO = (ORDER == 2 ? 0 : 1) + (SHIFTED ? 1 : 0);
   static constexpr int HHI = (ORDER == 2 ? 1 : 2);
   // largest value of the 3-D kernel: W(0)^3 = 1 (CIC), (3/4)^3 (TSC), (2/3)^3 (PCS)
@@ -70,6 +72,7 @@ struct PMTraits {
 template <int W>
 struct ESTraits {
   static constexpr int P = W;
+  static constexpr bool SHIFT = false;
   static constexpr bool ODD = (W & 1) != 0;
   static constexpr int HLO = ODD ? (W - 1) / 2 : W / 2 - 1;
   static constexpr int HHI = ODD ? (W + 1) / 2 : W / 2;
@@ -142,15 +145,6 @@ struct TMapSet {
   CUtensorMap m[N];
 };
 
-__device__ __forceinline__ int wrap(int v, int m) {  // general (slow: integer division by a run-time m)
-  v %= m;
-  return v < 0 ? v + m : v;
-}
-__device__ __forceinline__ int wrap_up(int v, int m) {  // v >= 0, a few multiples of m at most
-  while (v >= m) v -= m;
-  return v;
-}
-
 __device__ __forceinline__ void red_add_v4(float* addr, float4 v) {
   asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(v.x), "f"(v.y), "f"(v.z),
                "f"(v.w)
@@ -162,43 +156,89 @@ __device__ __forceinline__ float pow2i(int e) { return __int_as_float((e + 127) 
 struct TileOrigin {
   int x0, y0, z0;
 };
-__device__ __forceinline__ TileOrigin tile_origin(uint32_t tile, const BinView& bv) {  // inverse of tile_id()
+__device__ __forceinline__ TileOrigin tile_origin(const WorkItem& wi) {  // k_items packed the tile coordinates
   TileOrigin o;
-  const int tz = (int)(tile % (uint32_t)bv.ntz);
-  int r = (int)(tile / (uint32_t)bv.ntz);
-  const int xl = r & ((1 << bv.xbl) - 1);
-  r >>= bv.xbl;
-  o.z0 = tz * TZ;
-  o.y0 = (r % bv.nty) * TY;
-  o.x0 = (((r / bv.nty) << bv.xbl) | xl) * TX;
+  o.x0 = (int)(wi.txyz & 1023u) * TX;
+  o.y0 = (int)((wi.txyz >> 10) & 1023u) * TY;
+  o.z0 = (int)(wi.txyz >> 20) * TZ;
   return o;
+}
+__device__ __forceinline__ int wrap_lo(int v, int m) {                               // v in [-2m, m)
+  v += v < 0 ? m : 0;
+  v += v < 0 ? m : 0;
+  return v;
+}
+__device__ __forceinline__ int wrap_hi(int v, int m) {                               // v in [0, 3m)
+  v -= v >= m ? m : 0;
+  v -= v >= m ? m : 0;
+  return v;
 }
 
 // Subtract the fractional shift from a record coordinate (both REC_FRAC fixed point; rec carries REC_BIAS).
-__device__ __forceinline__ uint32_t apply_shift(uint32_t rec, uint32_t frac) { return rec - frac; }
+template <class T>
+__device__ __forceinline__ uint32_t apply_shift(uint32_t rec, uint32_t frac) {
+  return T::SHIFT ? rec - frac : rec;
+}
+
+// Dynamic tile schedule of the persistent scatter / gather kernels.  A CTA starts with item blockIdx.x and
+// then draws item ids from a global counter, so the items in flight are always a compact window of
+// consecutive tiles: the halo planes two neighbouring tiles share are touched close together in time and
+// are served from L2.  (A static stride lets CTAs drift apart: ncu showed the TMA halo reads of the gather
+// all going to DRAM.)  The last CTA to finish zeroes both counters for the next launch on the stream.
+__device__ __forceinline__ uint32_t sched_next(uint32_t* sched) { return gridDim.x + atomicAdd(&sched[0], 1u); }
+__device__ __forceinline__ void sched_done(uint32_t* sched) {
+  if (atomicAdd(&sched[1], 1u) == gridDim.x - 1u) {
+    sched[0] = 0u;
+    sched[1] = 0u;
+  }
+}
+
+// record loads: read once per kernel -> streaming (evict-first) so they do not push mesh tiles out of L2
+__device__ __forceinline__ uint4 load_rec(const uint4* p) { return __ldcs(p); }
 
 // ---- K2 / K5: tile scatter ---------------------------------------------------------------------------
-// Persistent CTAs loop over work items.  The accumulator tile is zeroed once; every flush writes zeros
-// back, so a work item costs two barriers.  roll is in [0, m).
+// Persistent CTAs draw work items from the dynamic schedule.  The accumulator tile is zeroed once; every
+// flush writes zeros back, so a work item costs two barriers.  roll is in [0, m).
 template <class T, int NCOMP, bool WEIGHTED>
 __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Params tp, int3 roll,
                                                    const float* __restrict__ wsrc, int wstride,
                                                    MeshPtrs<NCOMP> mesh) {
   using G = Geo<T>;
   constexpr int P = T::P;
+  constexpr int QZ = G::SZ / 4;                                 // float4 groups per z row
+  constexpr int NG = NCOMP * G::NGROUP;                          // groups to flush
+  constexpr int NSLOT = (NG + BLOCK - 1) / BLOCK;                // groups per thread
+  constexpr bool PRE = NSLOT <= 6;                               // group coordinates kept in registers
   extern __shared__ __align__(16) int s_acc[];
   __shared__ float s_red[(BLOCK / 32) * NCOMP];
+  __shared__ uint32_t s_next[2];
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
 
   for (int j = tid; j < NCOMP * G::PLANE / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
+
+  // (comp, sx, sy, 4q) of the groups this thread flushes, packed 4 | 8 | 8 | 12 bits
+  auto group_coords = [](int j) -> uint32_t {
+    const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
+    const int row = rr / QZ, q = rr - row * QZ;
+    const int sx = row / G::SY, sy = row - sx * G::SY;
+    return (uint32_t)(4 * q) | ((uint32_t)sy << 12) | ((uint32_t)sx << 20) | ((uint32_t)comp << 28);
+  };
+  uint32_t gc[PRE ? NSLOT : 1];
+  if (PRE) {
+#pragma unroll
+    for (int k = 0; k < NSLOT; ++k) gc[k] = group_coords(min(tid + k * BLOCK, NG - 1));
+  }
   __syncthreads();
 
-  for (uint32_t it = blockIdx.x; it < nitems; it += gridDim.x) {
+  uint32_t it = blockIdx.x;
+  int par = 0;
+  while (it < nitems) {
+    if (tid == 0) s_next[par] = sched_next(bv.sched);
     const WorkItem wi = bv.items[it];
     const uint32_t n = wi.end - wi.begin;
-    const TileOrigin o = tile_origin(wi.tile, bv);
+    const TileOrigin o = tile_origin(wi);
 
     // particles of this item -> registers
     uint4 r[PPT];
@@ -210,7 +250,7 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
     for (int k = 0; k < PPT; ++k) {
       const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
       if (i < wi.end) {
-        r[k] = bv.rec[i];
+        r[k] = load_rec(bv.rec + i);
 #pragma unroll
         for (int a = 0; a < NCOMP; ++a) {
           wv[k][a] = WEIGHTED ? __ldg(wsrc + (size_t)r[k].w * wstride + a) : 1.0f;
@@ -264,30 +304,30 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
       if (i < wi.end) {
         int sx, sy, sz;
         float wx[P], wy[P], wz[P], dummy[P];
-        T::template axis<false>(apply_shift(r[k].x, tp.frac[0]), tp, sx, wx, dummy);
-        T::template axis<false>(apply_shift(r[k].y, tp.frac[1]), tp, sy, wy, dummy);
-        T::template axis<false>(apply_shift(r[k].z, tp.frac[2]), tp, sz, wz, dummy);
+        T::template axis<false>(apply_shift<T>(r[k].x, tp.frac[0]), tp, sx, wx, dummy);
+        T::template axis<false>(apply_shift<T>(r[k].y, tp.frac[1]), tp, sy, wy, dummy);
+        T::template axis<false>(apply_shift<T>(r[k].z, tp.frac[2]), tp, sz, wz, dummy);
         sz += G::ZLO - G::HLO;
-        const int base = (sx * G::SY + sy) * G::SZ + sz;
-        float ws[NCOMP];
+        int* base = s_acc + (sx * G::SY + sy) * G::SZ + sz;
+        float wzs[NCOMP][P];  // the scale (and the particle's weight) folded into the z weights
 #pragma unroll
-        for (int a = 0; a < NCOMP; ++a) ws[a] = wv[k][a] * scale[a];
+        for (int q = 0; q < NCOMP; ++q)
+#pragma unroll
+          for (int c = 0; c < P; ++c) wzs[q][c] = wz[c] * (wv[k][q] * scale[q]);
 #pragma unroll
         for (int a = 0; a < P; ++a)
 #pragma unroll
           for (int b = 0; b < P; ++b) {
             const float wxy = wx[a] * wy[b];
-            const int row = base + (a * G::SY + b) * G::SZ;
+            int* row = base + (a * G::SY + b) * G::SZ;
 #pragma unroll
             for (int c = 0; c < P; ++c) {
-              const float wxyz = wxy * wz[c];
 #pragma unroll
               for (int q = 0; q < NCOMP; ++q) {
                 if (WEIGHTED)
-                  atomicAdd(&s_acc[q * G::PLANE + row + c], __float2int_rn(ws[q] * wxyz));
+                  atomicAdd(row + q * G::PLANE + c, __float2int_rn(wxy * wzs[q][c]));
                 else
-                  atomicAdd(reinterpret_cast<unsigned*>(&s_acc[q * G::PLANE + row + c]),
-                            __float2uint_rn(ws[q] * wxyz));
+                  atomicAdd(reinterpret_cast<unsigned*>(row + q * G::PLANE + c), __float2uint_rn(wxy * wzs[q][c]));
               }
             }
           }
@@ -296,43 +336,47 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
     __syncthreads();
 
     // flush: vectorised global reductions along z (red.global.add.v4.f32), empty groups skipped; the
-    // accumulators are zeroed on the way out.  bx/by/bz >= 0 so one conditional subtraction wraps.
-    const int bx = wrap(o.x0 - G::HLO - roll.x, m), by = wrap(o.y0 - G::HLO - roll.y, m);
-    const int bz = wrap(o.z0 - G::ZLO - roll.z, m);
-    for (int j = tid; j < NCOMP * G::NGROUP; j += BLOCK) {
-      const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
-      int4* src = reinterpret_cast<int4*>(s_acc) + comp * (G::PLANE / 4) + rr;
-      const int4 v = *src;
-      if ((v.x | v.y | v.z | v.w) == 0) continue;
-      *src = make_int4(0, 0, 0, 0);
-      const int q = rr % (G::SZ / 4), row = rr / (G::SZ / 4);
-      const int sy = row % G::SY, sx = row / G::SY;
-      float4 f;
-      if (WEIGHTED) {
+    // accumulators are zeroed on the way out.
+    const int bx = wrap_lo(o.x0 - G::HLO - roll.x, m), by = wrap_lo(o.y0 - G::HLO - roll.y, m);
+    const int bz = wrap_lo(o.z0 - G::ZLO - roll.z, m);
+#pragma unroll
+    for (int k = 0; k < (PRE ? NSLOT : 1); ++k) {
+      for (int j = tid + k * BLOCK; j < (PRE ? min(NG, (k + 1) * BLOCK) : NG); j += BLOCK) {
+        int4* src = reinterpret_cast<int4*>(s_acc) + j;  // PLANE / 4 == NGROUP: j indexes the groups directly
+        const int4 v = *src;
+        if ((v.x | v.y | v.z | v.w) == 0) continue;
+        *src = make_int4(0, 0, 0, 0);
+        const uint32_t g = PRE ? gc[k] : group_coords(j);
+        const int comp = NCOMP == 1 ? 0 : (int)(g >> 28);
         float is = inv_scale[0];
 #pragma unroll
         for (int a = 1; a < NCOMP; ++a)
           if (comp == a) is = inv_scale[a];
-        f = make_float4(__int2float_rn(v.x) * is, __int2float_rn(v.y) * is, __int2float_rn(v.z) * is,
-                        __int2float_rn(v.w) * is);
-      } else {
-        const float is = inv_scale[0];
-        f = make_float4(__uint2float_rn((unsigned)v.x) * is, __uint2float_rn((unsigned)v.y) * is,
-                        __uint2float_rn((unsigned)v.z) * is, __uint2float_rn((unsigned)v.w) * is);
-      }
-      const int gx = wrap_up(bx + sx, m), gy = wrap_up(by + sy, m), gz = wrap_up(bz + 4 * q, m);
-      float* p = mesh.p[comp] + ((size_t)gx * m + gy) * m;
-      if ((gz & 3) == 0) {
-        red_add_v4(p + gz, f);
-      } else {  // integer part of the shift not a multiple of 4: scalar reductions, each wrapped
-        atomicAdd(p + gz, f.x);
-        atomicAdd(p + wrap_up(gz + 1, m), f.y);
-        atomicAdd(p + wrap_up(gz + 2, m), f.z);
-        atomicAdd(p + wrap_up(gz + 3, m), f.w);
+        float4 f;
+        if (WEIGHTED)
+          f = make_float4(__int2float_rn(v.x) * is, __int2float_rn(v.y) * is, __int2float_rn(v.z) * is,
+                          __int2float_rn(v.w) * is);
+        else
+          f = make_float4(__uint2float_rn((unsigned)v.x) * is, __uint2float_rn((unsigned)v.y) * is,
+                          __uint2float_rn((unsigned)v.z) * is, __uint2float_rn((unsigned)v.w) * is);
+        const int gx = wrap_hi(bx + (int)((g >> 20) & 255u), m), gy = wrap_hi(by + (int)((g >> 12) & 255u), m);
+        const int gz = wrap_hi(bz + (int)(g & 4095u), m);
+        float* p = mesh.p[comp] + (size_t)(unsigned)(gx * m + gy) * (unsigned)m;
+        if ((gz & 3) == 0) {
+          red_add_v4(p + gz, f);
+        } else {  // integer part of the shift not a multiple of 4: scalar reductions, each wrapped
+          atomicAdd(p + gz, f.x);
+          atomicAdd(p + wrap_hi(gz + 1, m), f.y);
+          atomicAdd(p + wrap_hi(gz + 2, m), f.z);
+          atomicAdd(p + wrap_hi(gz + 3, m), f.w);
+        }
       }
     }
     __syncthreads();
+    it = s_next[par];
+    par ^= 1;
   }
+  if (tid == 0) sched_done(bv.sched);
 }
 
 // ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) --------------------------------------
@@ -359,11 +403,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   } while (!ok);
 }
 // box (innermost first) at coordinates (c0, c1, c2) = (z, y, x); out-of-bounds elements are zero-filled
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
+                                            uint64_t policy) {
+  if (policy == 0) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+    return;
+  }
   asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%3, %4, %5}], [%2], %6;"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
       : "memory");
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
 }
 
 // ---- K4 / K7: tile gather ----------------------------------------------------------------------------
@@ -371,8 +429,9 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 // GRAD = true : v[i*3 + b]     = sum_a coef_a(i) sum_j mesh_a[j] d/du_b W_j(X_i)             (Eq. C.6, C.12)
 // out = alpha * v (+ out if accumulate); the caller folds 1/Delta (d/dX = (1/Delta) d/du) into alpha.
 //
-// Persistent CTAs loop over work items.  Thread 0 stages the tile + halo box of every component with one
-// TMA tensor copy each (north_star "TMA staging of mesh tiles"), completion on an mbarrier; with STAGES = 2
+// Persistent CTAs draw work items from the dynamic schedule.  Thread 0 stages the tile + halo box of every
+// component with one TMA tensor copy each (north_star "TMA staging of mesh tiles"), completion on an
+// mbarrier, L2 evict-last hint (the halo planes are read again by the neighbouring tiles); with STAGES = 2
 // the box of the CTA's next item is in flight while the particles of the current one are interpolated.
 // TMA zero-fills what lies beyond the mesh edge, it does not wrap: tiles whose box crosses an edge (a few
 // per cent) are patched by the threads with periodic loads after the copy has landed.  roll in [0, m); when
@@ -388,46 +447,55 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   constexpr int P = T::P;
   constexpr int KB = 4;  // records in flight per thread
   constexpr uint32_t BOX_BYTES = (uint32_t)(NCOMP * G::PLANE * sizeof(float));
-  extern __shared__ unsigned char s_raw[];
+  extern __shared__ __align__(128) unsigned char s_raw[];
   __shared__ __align__(8) uint64_t s_bar[STAGES];
-  float* s_base = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(s_raw) + 127) & ~(uintptr_t)127);
+  __shared__ uint32_t s_next[2];
+  // 128-byte aligned TMA destinations; the offset is applied to the shared-space pointer so that the loads
+  // below stay LDS (a round trip through uintptr_t made them generic LD with 64-bit address arithmetic)
+  float* s_base = reinterpret_cast<float*>(s_raw + ((128u - (smem_u32(s_raw) & 127u)) & 127u));
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
 
+  uint64_t policy = 0;
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < STAGES; ++s) mbar_init(&s_bar[s], 1);
     fence_barrier_init();
     fence_proxy_async();
+    if (manual >> 1) policy = l2_policy_evict_last();
   }
   __syncthreads();
 
   auto box_start = [&](const TileOrigin& o, int& cx, int& cy, int& cz) {
-    cx = wrap(o.x0 - G::HLO - roll.x, m);
-    cy = wrap(o.y0 - G::HLO - roll.y, m);
-    cz = wrap(o.z0 - G::ZLO - roll.z, m);
+    cx = wrap_lo(o.x0 - G::HLO - roll.x, m);
+    cy = wrap_lo(o.y0 - G::HLO - roll.y, m);
+    cz = wrap_lo(o.z0 - G::ZLO - roll.z, m);
   };
   auto issue = [&](uint32_t item, int stage) {  // thread 0
-    if (manual) return;
-    const TileOrigin o = tile_origin(bv.items[item].tile, bv);
+    if (manual & 1) return;
+    const TileOrigin o = tile_origin(bv.items[item]);
     int cx, cy, cz;
     box_start(o, cx, cy, cz);
     mbar_expect_tx(&s_bar[stage], BOX_BYTES);
 #pragma unroll
     for (int a = 0; a < NCOMP; ++a)
-      tma_load_3d(s_base + (stage * NCOMP + a) * G::PLANE_PAD, &maps.m[a], &s_bar[stage], cz, cy, cx);
+      tma_load_3d(s_base + (stage * NCOMP + a) * G::PLANE_PAD, &maps.m[a], &s_bar[stage], cz, cy, cx, policy);
   };
 
   uint32_t phases = 0;  // bit s: parity the next wait on stage s uses
-  int stage = 0;
-  if (tid == 0 && blockIdx.x < nitems) issue(blockIdx.x, 0);
+  int stage = 0, par = 0;
+  uint32_t it = blockIdx.x;
+  if (tid == 0 && it < nitems) issue(it, 0);
 
-  for (uint32_t it = blockIdx.x; it < nitems; it += gridDim.x) {
-    const uint32_t next = it + gridDim.x;
-    if (STAGES == 2 && tid == 0 && next < nitems) issue(next, stage ^ 1);
+  while (it < nitems) {
+    if (tid == 0) {
+      const uint32_t next = sched_next(bv.sched);
+      s_next[par] = next;
+      if (STAGES == 2 && next < nitems) issue(next, stage ^ 1);
+    }
     const WorkItem wi = bv.items[it];
-    const TileOrigin o = tile_origin(wi.tile, bv);
+    const TileOrigin o = tile_origin(wi);
     const float* s_val = s_base + stage * NCOMP * G::PLANE_PAD;
 
     // first batch of records: in flight while the box lands
@@ -435,27 +503,27 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
     for (int k = 0; k < KB; ++k) {
       const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
-      if (i < wi.end) r[k] = bv.rec[i];
+      if (i < wi.end) r[k] = load_rec(bv.rec + i);
     }
 
-    if (!manual) {
+    if (!(manual & 1)) {
       mbar_wait(&s_bar[stage], (phases >> stage) & 1u);
       phases ^= 1u << stage;
     }
 
     int cx, cy, cz;
     box_start(o, cx, cy, cz);
-    if (manual || cx + G::SX > m || cy + G::SY > m || cz + G::SZ > m) {  // uniform: box crosses a mesh edge
+    if ((manual & 1) || cx + G::SX > m || cy + G::SY > m || cz + G::SZ > m) {  // uniform: box crosses a mesh edge
       float* s_w = s_base + stage * NCOMP * G::PLANE_PAD;
       for (int j = tid; j < NCOMP * G::NGROUP; j += BLOCK) {
         const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
         const int q = rr % (G::SZ / 4), row = rr / (G::SZ / 4);
         const int sy = row % G::SY, sx = row / G::SY;
-        if (!manual && cx + sx < m && cy + sy < m && cz + 4 * q + 3 < m) continue;  // TMA delivered it
-        const float* p = mesh.p[comp] + ((size_t)wrap_up(cx + sx, m) * m + wrap_up(cy + sy, m)) * m;
+        if (!(manual & 1) && cx + sx < m && cy + sy < m && cz + 4 * q + 3 < m) continue;  // TMA delivered it
+        const float* p = mesh.p[comp] + ((size_t)wrap_hi(cx + sx, m) * m + wrap_hi(cy + sy, m)) * m;
         const int gz = cz + 4 * q;
-        const float4 v = make_float4(__ldg(p + wrap_up(gz, m)), __ldg(p + wrap_up(gz + 1, m)),
-                                     __ldg(p + wrap_up(gz + 2, m)), __ldg(p + wrap_up(gz + 3, m)));
+        const float4 v = make_float4(__ldg(p + wrap_hi(gz, m)), __ldg(p + wrap_hi(gz + 1, m)),
+                                     __ldg(p + wrap_hi(gz + 2, m)), __ldg(p + wrap_hi(gz + 3, m)));
         reinterpret_cast<float4*>(s_w + comp * G::PLANE_PAD)[rr] = v;
       }
       fence_proxy_async();  // generic-proxy writes before the async proxy refills this buffer
@@ -467,7 +535,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
         for (int k = 0; k < KB; ++k) {
           const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
-          if (i < wi.end) r[k] = bv.rec[i];
+          if (i < wi.end) r[k] = load_rec(bv.rec + i);
         }
       }
 #pragma unroll
@@ -477,11 +545,11 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         const uint4 rk = r[k];
         int sx, sy, sz;
         float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
-        T::template axis<GRAD>(apply_shift(rk.x, tp.frac[0]), tp, sx, wx, dx);
-        T::template axis<GRAD>(apply_shift(rk.y, tp.frac[1]), tp, sy, wy, dy);
-        T::template axis<GRAD>(apply_shift(rk.z, tp.frac[2]), tp, sz, wz, dz);
+        T::template axis<GRAD>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
+        T::template axis<GRAD>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
+        T::template axis<GRAD>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
         sz += G::ZLO - G::HLO;
-        const int base = (sx * G::SY + sy) * G::SZ + sz;
+        const float* base = s_val + (sx * G::SY + sy) * G::SZ + sz;
         if (!GRAD) {
           float acc[NCOMP];
 #pragma unroll
@@ -491,12 +559,12 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
             for (int b = 0; b < P; ++b) {
               const float wxy = wx[a] * wy[b];
-              const int row = base + (a * G::SY + b) * G::SZ;
+              const float* row = base + (a * G::SY + b) * G::SZ;
 #pragma unroll
               for (int c = 0; c < P; ++c) {
                 const float wxyz = wxy * wz[c];
 #pragma unroll
-                for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, s_val[q * G::PLANE_PAD + row + c], acc[q]);
+                for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, row[q * G::PLANE_PAD + c], acc[q]);
               }
             }
 #pragma unroll
@@ -514,13 +582,13 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
           for (int a = 0; a < P; ++a)
 #pragma unroll
             for (int b = 0; b < P; ++b) {
-              const int row = base + (a * G::SY + b) * G::SZ;
+              const float* row = base + (a * G::SY + b) * G::SZ;
               const float wdx = dx[a] * wy[b], wdy = wx[a] * dy[b], wxy = wx[a] * wy[b];
 #pragma unroll
               for (int c = 0; c < P; ++c) {
                 float val = 0.0f;
 #pragma unroll
-                for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], s_val[q * G::PLANE_PAD + row + c], val);
+                for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], row[q * G::PLANE_PAD + c], val);
                 gx = fmaf(wdx * wz[c], val, gx);
                 gy = fmaf(wdy * wz[c], val, gy);
                 gz = fmaf(wxy * dz[c], val, gz);
@@ -534,15 +602,22 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
       }
     }
     __syncthreads();  // every thread is done with this stage: it may be refilled
+    it = s_next[par];
+    par ^= 1;
     if (STAGES == 2) {
       stage ^= 1;
-    } else if (tid == 0 && next < nitems) {
-      issue(next, 0);
+    } else if (tid == 0 && it < nitems) {
+      issue(it, 0);
     }
   }
+  if (tid == 0) sched_done(bv.sched);
 }
 
 // ---- host-side launch helpers ------------------------------------------------------------------------
+inline int tune_flag(const char* name, int dflt) {  // tuning knobs read once from the environment
+  const char* v = getenv(name);
+  return v ? atoi(v) : dflt;
+}
 inline int norm_roll(int r, int m) {
   r %= m;
   return r < 0 ? r + m : r;
@@ -603,7 +678,7 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const fl
   const float a_eff = GRAD ? (float)((double)alpha * (double)c->mg / c->p.box) : alpha;
   const int3 nr = make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m));
   kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp, nr, maps, mp, cot, cstride, ncot, const_coef, wmul,
-                                               a_eff, accumulate ? 1 : 0, (nr.z & 3) ? 1 : 0, out);
+                                               a_eff, accumulate ? 1 : 0, ((nr.z & 3) ? 1 : 0) | (tune_flag("PMF_TMA_EVICT_LAST", 0) << 1), out);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

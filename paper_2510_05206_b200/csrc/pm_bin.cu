@@ -69,30 +69,61 @@ __device__ __forceinline__ uint32_t tile_only(float x, float y, float z, const B
 }
 
 // The lanes of a warp hold 32 CONSECUTIVE particles.  Each run of equal keys elects its first lane, which
-// performs ONE atomic for the run; returns the slot of this lane (run base + rank in the run), so that a
-// coherent input (Lagrangian order) keeps its order inside a tile -- the scatter / gather kernels rely on
-// that for conflict-free shared-memory access.  Lanes with valid = false take no slot.
-__device__ __forceinline__ uint32_t warp_claim(uint32_t* counters, uint32_t key, bool valid) {
+// performs ONE atomic for the run; a lane's slot is run base + rank in the run, so that a coherent input
+// (Lagrangian order) keeps its order inside a tile -- the scatter / gather kernels rely on that for
+// conflict-free shared-memory access.  Lanes whose key is NO_TILE take no slot.
+struct Claim {
+  int head;       // lane that performs the atomic of this lane's run
+  uint32_t len;   // run length (meaningful on the head lane)
+  uint32_t rank;  // this lane's position in its run
+};
+__device__ __forceinline__ Claim warp_runs(uint32_t key) {
   const unsigned lane = threadIdx.x & 31u;
-  if (!valid) key = 0xffffffffu;
   const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
   const unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || key != prev);
-  const unsigned le = heads & (0xffffffffu >> (31u - lane));   // heads at or below this lane
-  const int head = 31 - __clz(le);
+  const unsigned le = heads & (0xffffffffu >> (31u - lane));  // heads at or below this lane
   const unsigned above = heads & ~(0xffffffffu >> (31u - lane));
-  const int next = above ? __ffs(above) - 1 : 32;
-  uint32_t base = 0;
-  if (valid && (int)lane == head) base = atomicAdd(&counters[key], (uint32_t)(next - (int)lane));
-  base = __shfl_sync(0xffffffffu, base, head);
-  return base + (lane - (unsigned)head);
+  Claim c;
+  c.head = 31 - __clz(le);
+  c.len = (uint32_t)((above ? __ffs(above) - 1 : 32) - c.head);
+  c.rank = lane - (unsigned)c.head;
+  return c;
 }
 
 constexpr int BIN_BLOCK = 256;
 constexpr int BIN_WARP_PART = 128;  // particles per warp and iteration (3 float4 per lane)
+constexpr uint32_t NO_TILE = 0xffffffffu;
+
+// Claim slots for K keys per lane at once: the K atomics of a lane are issued back to back and only then
+// consumed, so their round trips to L2 overlap (issued one by one, each claim waited for the previous).
+template <bool PERMUTE, int K>
+__device__ __forceinline__ void claim_slots(uint32_t* __restrict__ counters, const uint32_t (&key)[K],
+                                            uint32_t (&slot)[K]) {
+  const unsigned lane = threadIdx.x & 31u;
+  Claim c[K];
+  uint32_t base[K];
+#pragma unroll
+  for (int k = 0; k < K; ++k) c[k] = warp_runs(key[k]);
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    base[k] = 0;
+    if ((int)lane == c[k].head && key[k] != NO_TILE) {
+      if (PERMUTE)
+        base[k] = atomicAdd(&counters[key[k]], c[k].len);
+      else
+        atomicAdd(&counters[key[k]], c[k].len);  // histogram only: no return value (RED)
+    }
+  }
+  if (PERMUTE) {
+#pragma unroll
+    for (int k = 0; k < K; ++k) slot[k] = __shfl_sync(0xffffffffu, base[k], c[k].head) + c[k].rank;
+  }
+}
 
 // pass 1 (PERMUTE = false): tile histogram; pass 2 (PERMUTE = true): claim a slot, store the record.
 // Positions are read as coalesced float4 (north_star "coalesced float4 position loads") and transposed
-// through a warp-private shared-memory strip so that lane l handles particles 32k + l, k = 0..3.
+// through a warp-private shared-memory strip so that lane l handles particles 32k + l, k = 0..3; the next
+// chunk's loads are in flight while the current one is processed.
 template <bool PERMUTE>
 __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict__ pos, int64_t n, BinGeom g,
                                                         uint32_t* __restrict__ counters,
@@ -105,21 +136,35 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
   const int64_t gwarp = (int64_t)blockIdx.x * (BIN_BLOCK / 32) + warp;
   const int64_t nwarps = (int64_t)gridDim.x * (BIN_BLOCK / 32);
   const float4* p4 = reinterpret_cast<const float4*>(pos);
+  float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
+  if (gwarp < nchunk) {
+    const float4* src = p4 + gwarp * (BIN_WARP_PART * 3 / 4);
+    a = __ldcs(src + lane), b = __ldcs(src + 32 + lane), c = __ldcs(src + 64 + lane);
+  }
   for (int64_t ch = gwarp; ch < nchunk; ch += nwarps) {
-    const float4* src = p4 + ch * (BIN_WARP_PART * 3 / 4);
-    const float4 a = __ldg(src + lane), b = __ldg(src + 32 + lane), c = __ldg(src + 64 + lane);
     reinterpret_cast<float4*>(s)[lane] = a;
     reinterpret_cast<float4*>(s)[32 + lane] = b;
     reinterpret_cast<float4*>(s)[64 + lane] = c;
     __syncwarp();
+    if (ch + nwarps < nchunk) {
+      const float4* src = p4 + (ch + nwarps) * (BIN_WARP_PART * 3 / 4);
+      a = __ldcs(src + lane), b = __ldcs(src + 32 + lane), c = __ldcs(src + 64 + lane);
+    }
+    uint32_t tile[4], slot[4], fx[4], fy[4], fz[4], toff[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       const int j = 32 * k + (int)lane;
       const float x = s[3 * j], y = s[3 * j + 1], z = s[3 * j + 2];
-      uint32_t fx = 0, fy = 0, fz = 0;
-      const uint32_t tile = PERMUTE ? tile_and_local(x, y, z, g, fx, fy, fz) : tile_only(x, y, z, g);
-      const uint32_t slot = warp_claim(counters, tile, true);
-      if (PERMUTE) rec[tile_off[tile] + slot] = make_uint4(fx, fy, fz, (uint32_t)(ch * BIN_WARP_PART + j));
+      fx[k] = fy[k] = fz[k] = 0;
+      tile[k] = PERMUTE ? tile_and_local(x, y, z, g, fx[k], fy[k], fz[k]) : tile_only(x, y, z, g);
+      if (PERMUTE) toff[k] = __ldg(tile_off + tile[k]);
+    }
+    claim_slots<PERMUTE, 4>(counters, tile, slot);
+    if (PERMUTE) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        rec[toff[k] + slot[k]] =
+            make_uint4(fx[k], fy[k], fz[k], (uint32_t)(ch * BIN_WARP_PART + 32 * k + (int)lane));
     }
     __syncwarp();
   }
@@ -129,14 +174,15 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
   const int64_t rest_round = (rest + 31) / 32 * 32;
   for (int64_t j = gwarp * 32 + lane; j < rest_round; j += nwarps * 32) {
     const bool valid = j < rest;
-    uint32_t fx = 0, fy = 0, fz = 0, tile = 0;
+    uint32_t fx = 0, fy = 0, fz = 0;
+    uint32_t tile[1] = {NO_TILE}, slot[1] = {0};
     const int64_t i = first + j;
     if (valid) {
       const float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
-      tile = PERMUTE ? tile_and_local(x, y, z, g, fx, fy, fz) : tile_only(x, y, z, g);
+      tile[0] = PERMUTE ? tile_and_local(x, y, z, g, fx, fy, fz) : tile_only(x, y, z, g);
     }
-    const uint32_t slot = warp_claim(counters, tile, valid);
-    if (PERMUTE && valid) rec[tile_off[tile] + slot] = make_uint4(fx, fy, fz, (uint32_t)i);
+    claim_slots<PERMUTE, 1>(counters, tile, slot);
+    if (PERMUTE && valid) rec[tile_off[tile[0]] + slot[0]] = make_uint4(fx, fy, fz, (uint32_t)i);
   }
 }
 

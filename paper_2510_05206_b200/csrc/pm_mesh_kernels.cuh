@@ -111,26 +111,54 @@ struct ESTraits {
   }
 };
 
-// Shared-memory tile geometry.  The z origin of a staged tile is 4-aligned (ZLO = HLO rounded up): the scatter
-// flushes with 16-byte vector reductions and a TMA box must start on a 16-byte boundary of the innermost
-// dimension (measured: an unaligned start coordinate raises "illegal instruction" on sm_100a).
+// Shared-memory tile geometry.  A staged tile covers nodes [x0 - HLO, x0 + TX + HHI) x [y0 - HLO, ...) and, along
+// z, [z0 - ZLO, z0 - ZLO + TZ + HZ) with ZLO = HLO rounded up to 4 (16-byte vector reductions, and a TMA box
+// must start on a 16-byte boundary of the innermost dimension: an unaligned start coordinate raises "illegal
+// instruction" on sm_100a).  Each (x, y) row is stored in two pieces: the first TZ = 32 nodes in the MAIN plane
+// with a row pitch of exactly 32 words, the remaining HZ (4 or 8) in the HALO plane.  With a pitch of 32 the
+// bank of a main-plane node is its z index alone, so a warp whose 32 lanes hold particles at 32 different z
+// (one lattice row in Lagrangian order) is conflict-free whatever their (x, y) cells are; a dense pitch of
+// TZ + halo made every access a 2-way conflict (ncu: 51 % of the shared wavefronts).
 template <class T>
 struct Geo {
   static constexpr int P = T::P, HLO = T::HLO, HHI = T::HHI;
-  static constexpr int ZLO = (HLO + 3) / 4 * 4, ZHI = (HHI + 3) / 4 * 4;
-  static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, SZ = TZ + ZLO + ZHI;
-  static constexpr int PLANE = SX * SY * SZ;         // smem words per component
-  static constexpr int NGROUP = SX * SY * (SZ / 4);  // float4 groups per component
-};
-template <class T>
-struct GeoG {
-  static constexpr int P = T::P, HLO = T::HLO, HHI = T::HHI;
   static constexpr int ZLO = (HLO + 3) / 4 * 4;
-  static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, SZ = (ZLO + TZ + HHI + 3) / 4 * 4;
-  static constexpr int PLANE = SX * SY * SZ;             // box elements per component
-  static constexpr int PLANE_PAD = (PLANE + 31) / 32 * 32;  // TMA destinations are 128-byte aligned
-  static constexpr int NGROUP = SX * SY * (SZ / 4);
+  static constexpr int HZ = ZLO + (HHI + 3) / 4 * 4;                 // halo columns per row
+  static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, NROW = SX * SY;
+  static constexpr int MAIN = NROW * TZ, HAL = NROW * HZ;            // words per component
+  static constexpr int COMP = (MAIN + HAL + 31) / 32 * 32;           // component block (128-byte multiple)
+  static constexpr int NGM = NROW * (TZ / 4), NGH = NROW * (HZ / 4); // float4 groups per component
+  static constexpr int NGROUP = NGM + NGH;
+  static_assert(TZ == 32, "the main plane's row pitch must be 32 words");
+  static_assert(HZ == 4 || HZ == 8, "halo columns");
 };
+
+// Address of node column s (0 <= s < TZ + HZ, relative to the box start) in row `row` of a component block:
+//   s < TZ : MAIN[row * TZ + s]        else : HAL[row * HZ + s - TZ]
+// NodeCol holds the per-column part; the row part is one multiply-add (row * pitch + base).
+struct NodeCol {
+  int base, pitch;
+};
+template <class G>
+__device__ __forceinline__ NodeCol node_col(int row0, int s) {  // row0 = index of the particle's first row
+  NodeCol c;
+  const bool main = s < TZ;
+  c.pitch = main ? TZ : G::HZ;
+  c.base = main ? row0 * TZ + s : G::MAIN + row0 * G::HZ + (s - TZ);
+  return c;
+}
+// float4 group j of a component block -> (row, z offset of its first node relative to the box start)
+template <class G>
+__device__ __forceinline__ void group_pos(int j, int& row, int& zoff) {
+  if (j < G::NGM) {
+    row = j / (TZ / 4);
+    zoff = 4 * (j - row * (TZ / 4));
+  } else {
+    const int h = j - G::NGM;
+    row = h / (G::HZ / 4);
+    zoff = TZ + 4 * (h - row * (G::HZ / 4));
+  }
+}
 
 template <int N>
 struct MeshPtrs {
@@ -205,7 +233,6 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
                                                    MeshPtrs<NCOMP> mesh) {
   using G = Geo<T>;
   constexpr int P = T::P;
-  constexpr int QZ = G::SZ / 4;                                 // float4 groups per z row
   constexpr int NG = NCOMP * G::NGROUP;                          // groups to flush
   constexpr int NSLOT = (NG + BLOCK - 1) / BLOCK;                // groups per thread
   constexpr bool PRE = NSLOT <= 6;                               // group coordinates kept in registers
@@ -216,14 +243,15 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
 
-  for (int j = tid; j < NCOMP * G::PLANE / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
+  for (int j = tid; j < NCOMP * G::COMP / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
 
-  // (comp, sx, sy, 4q) of the groups this thread flushes, packed 4 | 8 | 8 | 12 bits
+  // (comp, sx, sy, z offset) of the groups this thread flushes, packed 4 | 8 | 8 | 12 bits
   auto group_coords = [](int j) -> uint32_t {
-    const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
-    const int row = rr / QZ, q = rr - row * QZ;
+    const int comp = j / G::NGROUP;
+    int row, zoff;
+    group_pos<G>(j - comp * G::NGROUP, row, zoff);
     const int sx = row / G::SY, sy = row - sx * G::SY;
-    return (uint32_t)(4 * q) | ((uint32_t)sy << 12) | ((uint32_t)sx << 20) | ((uint32_t)comp << 28);
+    return (uint32_t)zoff | ((uint32_t)sy << 12) | ((uint32_t)sx << 20) | ((uint32_t)comp << 28);
   };
   uint32_t gc[PRE ? NSLOT : 1];
   if (PRE) {
@@ -232,25 +260,35 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
   }
   __syncthreads();
 
+  // records of a work item -> registers.  The next item's records are requested right after the deposit
+  // loop, so their latency is covered by the flush of the current tile.
+  WorkItem wi;
+  uint4 r[PPT];
+  auto load_item = [&](uint32_t id) {
+    wi = bv.items[id];
+#pragma unroll
+    for (int k = 0; k < PPT; ++k) {
+      const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
+      if (i < wi.end) r[k] = load_rec(bv.rec + i);
+    }
+  };
   uint32_t it = blockIdx.x;
   int par = 0;
+  if (it < nitems) load_item(it);
   while (it < nitems) {
     if (tid == 0) s_next[par] = sched_next(bv.sched);
-    const WorkItem wi = bv.items[it];
     const uint32_t n = wi.end - wi.begin;
+    const uint32_t ibegin = wi.begin, iend = wi.end;
     const TileOrigin o = tile_origin(wi);
 
-    // particles of this item -> registers
-    uint4 r[PPT];
     float wv[PPT][NCOMP];
     float wabs[NCOMP];
 #pragma unroll
     for (int a = 0; a < NCOMP; ++a) wabs[a] = 0.0f;
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
-      const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
-      if (i < wi.end) {
-        r[k] = load_rec(bv.rec + i);
+      const uint32_t i = ibegin + (uint32_t)(k * BLOCK + tid);
+      if (i < iend) {
 #pragma unroll
         for (int a = 0; a < NCOMP; ++a) {
           wv[k][a] = WEIGHTED ? __ldg(wsrc + (size_t)r[k].w * wstride + a) : 1.0f;
@@ -300,15 +338,16 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
 
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
-      const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
-      if (i < wi.end) {
+      const uint32_t i = ibegin + (uint32_t)(k * BLOCK + tid);
+      if (i < iend) {
         int sx, sy, sz;
         float wx[P], wy[P], wz[P], dummy[P];
         T::template axis<false>(apply_shift<T>(r[k].x, tp.frac[0]), tp, sx, wx, dummy);
         T::template axis<false>(apply_shift<T>(r[k].y, tp.frac[1]), tp, sy, wy, dummy);
         T::template axis<false>(apply_shift<T>(r[k].z, tp.frac[2]), tp, sz, wz, dummy);
-        sz += G::ZLO - G::HLO;
-        int* base = s_acc + (sx * G::SY + sy) * G::SZ + sz;
+        NodeCol nc[P];
+#pragma unroll
+        for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
         float wzs[NCOMP][P];  // the scale (and the particle's weight) folded into the z weights
 #pragma unroll
         for (int q = 0; q < NCOMP; ++q)
@@ -319,21 +358,24 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
 #pragma unroll
           for (int b = 0; b < P; ++b) {
             const float wxy = wx[a] * wy[b];
-            int* row = base + (a * G::SY + b) * G::SZ;
 #pragma unroll
             for (int c = 0; c < P; ++c) {
+              int* node = s_acc + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
 #pragma unroll
               for (int q = 0; q < NCOMP; ++q) {
                 if (WEIGHTED)
-                  atomicAdd(row + q * G::PLANE + c, __float2int_rn(wxy * wzs[q][c]));
+                  atomicAdd(node + q * G::COMP, __float2int_rn(wxy * wzs[q][c]));
                 else
-                  atomicAdd(reinterpret_cast<unsigned*>(row + q * G::PLANE + c), __float2uint_rn(wxy * wzs[q][c]));
+                  atomicAdd(reinterpret_cast<unsigned*>(node + q * G::COMP), __float2uint_rn(wxy * wzs[q][c]));
               }
             }
           }
       }
     }
     __syncthreads();
+    it = s_next[par];
+    par ^= 1;
+    if (it < nitems) load_item(it);
 
     // flush: vectorised global reductions along z (red.global.add.v4.f32), empty groups skipped; the
     // accumulators are zeroed on the way out.
@@ -342,7 +384,8 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
 #pragma unroll
     for (int k = 0; k < (PRE ? NSLOT : 1); ++k) {
       for (int j = tid + k * BLOCK; j < (PRE ? min(NG, (k + 1) * BLOCK) : NG); j += BLOCK) {
-        int4* src = reinterpret_cast<int4*>(s_acc) + j;  // PLANE / 4 == NGROUP: j indexes the groups directly
+        const int jc = NCOMP == 1 ? 0 : j / G::NGROUP;  // component blocks are padded to COMP words
+        int4* src = reinterpret_cast<int4*>(s_acc) + (j + jc * (G::COMP / 4 - G::NGROUP));
         const int4 v = *src;
         if ((v.x | v.y | v.z | v.w) == 0) continue;
         *src = make_int4(0, 0, 0, 0);
@@ -373,8 +416,6 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
       }
     }
     __syncthreads();
-    it = s_next[par];
-    par ^= 1;
   }
   if (tid == 0) sched_done(bv.sched);
 }
@@ -438,15 +479,15 @@ __device__ __forceinline__ uint64_t l2_policy_evict_last() {
 // roll.z is not a multiple of 4 no box start is 16-byte aligned and the threads stage everything (manual).
 template <class T, int NCOMP, bool GRAD, int STAGES>
 __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params tp, int3 roll,
-                                                  const __grid_constant__ TMapSet<NCOMP> maps,
+                                                  const __grid_constant__ TMapSet<2 * NCOMP> maps,
                                                   CMeshPtrs<NCOMP> mesh, const float* __restrict__ cot,
                                                   int cstride, int ncot, float const_coef,
                                                   const float* __restrict__ wmul, float alpha,
                                                   int accumulate, int manual, float* __restrict__ out) {
-  using G = GeoG<T>;
+  using G = Geo<T>;
   constexpr int P = T::P;
   constexpr int KB = 4;  // records in flight per thread
-  constexpr uint32_t BOX_BYTES = (uint32_t)(NCOMP * G::PLANE * sizeof(float));
+  constexpr uint32_t BOX_BYTES = (uint32_t)(NCOMP * (G::MAIN + G::HAL) * sizeof(float));
   extern __shared__ __align__(128) unsigned char s_raw[];
   __shared__ __align__(8) uint64_t s_bar[STAGES];
   __shared__ uint32_t s_next[2];
@@ -479,8 +520,11 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     box_start(o, cx, cy, cz);
     mbar_expect_tx(&s_bar[stage], BOX_BYTES);
 #pragma unroll
-    for (int a = 0; a < NCOMP; ++a)
-      tma_load_3d(s_base + (stage * NCOMP + a) * G::PLANE_PAD, &maps.m[a], &s_bar[stage], cz, cy, cx, policy);
+    for (int a = 0; a < NCOMP; ++a) {  // main plane (first TZ nodes of every row) and halo plane (the rest)
+      float* dst = s_base + (stage * NCOMP + a) * G::COMP;
+      tma_load_3d(dst, &maps.m[2 * a], &s_bar[stage], cz, cy, cx, policy);
+      tma_load_3d(dst + G::MAIN, &maps.m[2 * a + 1], &s_bar[stage], cz + TZ, cy, cx, policy);
+    }
   };
 
   uint32_t phases = 0;  // bit s: parity the next wait on stage s uses
@@ -496,7 +540,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     }
     const WorkItem wi = bv.items[it];
     const TileOrigin o = tile_origin(wi);
-    const float* s_val = s_base + stage * NCOMP * G::PLANE_PAD;
+    const float* s_val = s_base + stage * NCOMP * G::COMP;
 
     // first batch of records: in flight while the box lands
     uint4 r[KB];
@@ -513,18 +557,19 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 
     int cx, cy, cz;
     box_start(o, cx, cy, cz);
-    if ((manual & 1) || cx + G::SX > m || cy + G::SY > m || cz + G::SZ > m) {  // uniform: box crosses a mesh edge
-      float* s_w = s_base + stage * NCOMP * G::PLANE_PAD;
+    if ((manual & 1) || cx + G::SX > m || cy + G::SY > m || cz + TZ + G::HZ > m) {  // uniform: box crosses a mesh edge
+      float* s_w = s_base + stage * NCOMP * G::COMP;
       for (int j = tid; j < NCOMP * G::NGROUP; j += BLOCK) {
         const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
-        const int q = rr % (G::SZ / 4), row = rr / (G::SZ / 4);
+        int row, zoff;
+        group_pos<G>(rr, row, zoff);
         const int sy = row % G::SY, sx = row / G::SY;
-        if (!(manual & 1) && cx + sx < m && cy + sy < m && cz + 4 * q + 3 < m) continue;  // TMA delivered it
+        if (!(manual & 1) && cx + sx < m && cy + sy < m && cz + zoff + 3 < m) continue;  // TMA delivered it
         const float* p = mesh.p[comp] + ((size_t)wrap_hi(cx + sx, m) * m + wrap_hi(cy + sy, m)) * m;
-        const int gz = cz + 4 * q;
+        const int gz = cz + zoff;
         const float4 v = make_float4(__ldg(p + wrap_hi(gz, m)), __ldg(p + wrap_hi(gz + 1, m)),
                                      __ldg(p + wrap_hi(gz + 2, m)), __ldg(p + wrap_hi(gz + 3, m)));
-        reinterpret_cast<float4*>(s_w + comp * G::PLANE_PAD)[rr] = v;
+        reinterpret_cast<float4*>(s_w + comp * G::COMP)[rr] = v;
       }
       fence_proxy_async();  // generic-proxy writes before the async proxy refills this buffer
       __syncthreads();
@@ -548,8 +593,9 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         T::template axis<GRAD>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
         T::template axis<GRAD>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
         T::template axis<GRAD>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
-        sz += G::ZLO - G::HLO;
-        const float* base = s_val + (sx * G::SY + sy) * G::SZ + sz;
+        NodeCol nc[P];
+#pragma unroll
+        for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
         if (!GRAD) {
           float acc[NCOMP];
 #pragma unroll
@@ -559,12 +605,12 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
             for (int b = 0; b < P; ++b) {
               const float wxy = wx[a] * wy[b];
-              const float* row = base + (a * G::SY + b) * G::SZ;
 #pragma unroll
               for (int c = 0; c < P; ++c) {
                 const float wxyz = wxy * wz[c];
+                const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
 #pragma unroll
-                for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, row[q * G::PLANE_PAD + c], acc[q]);
+                for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, node[q * G::COMP], acc[q]);
               }
             }
 #pragma unroll
@@ -582,13 +628,13 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
           for (int a = 0; a < P; ++a)
 #pragma unroll
             for (int b = 0; b < P; ++b) {
-              const float* row = base + (a * G::SY + b) * G::SZ;
               const float wdx = dx[a] * wy[b], wdy = wx[a] * dy[b], wxy = wx[a] * wy[b];
 #pragma unroll
               for (int c = 0; c < P; ++c) {
+                const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
                 float val = 0.0f;
 #pragma unroll
-                for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], row[q * G::PLANE_PAD + c], val);
+                for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], node[q * G::COMP], val);
                 gx = fmaf(wdx * wz[c], val, gx);
                 gy = fmaf(wdy * wz[c], val, gy);
                 gz = fmaf(wxy * dz[c], val, gz);
@@ -634,7 +680,7 @@ template <class T, int NCOMP, bool WEIGHTED>
 int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const float* wsrc, int wstride,
                 float* const mesh[], cudaStream_t st) {
   using G = Geo<T>;
-  const size_t smem = sizeof(int) * (size_t)NCOMP * G::PLANE;
+  const size_t smem = sizeof(int) * (size_t)NCOMP * G::COMP;
   auto kern = k_scatter<T, NCOMP, WEIGHTED>;
   static int occ = 0;
   if (!occ) {
@@ -657,8 +703,8 @@ template <class T, int NCOMP, bool GRAD>
 int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const float* const mesh[],
                const float* cot, int cstride, int ncot, float const_coef, const float* wmul, float alpha,
                bool accumulate, float* out, cudaStream_t st) {
-  using G = GeoG<T>;
-  constexpr size_t stage_bytes = sizeof(float) * (size_t)NCOMP * G::PLANE_PAD;
+  using G = Geo<T>;
+  constexpr size_t stage_bytes = sizeof(float) * (size_t)NCOMP * G::COMP;
   constexpr int STAGES = 2 * stage_bytes <= 100 * 1024 ? 2 : 1;
   constexpr size_t smem = STAGES * stage_bytes + 128;
   auto kern = k_gather<T, NCOMP, GRAD, STAGES>;
@@ -669,11 +715,12 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const fl
     if (occ < 1) return fail(c, PM_ECUDA, "gather kernel does not fit on an SM");
   }
   CMeshPtrs<NCOMP> mp;
-  TMapSet<NCOMP> maps;
+  TMapSet<2 * NCOMP> maps;
   const int m = c->mg;
   for (int a = 0; a < NCOMP; ++a) {
     mp.p[a] = mesh[a];
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::SZ, &maps.m[a]));
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, &maps.m[2 * a]));
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::HZ, &maps.m[2 * a + 1]));
   }
   const float a_eff = GRAD ? (float)((double)alpha * (double)c->mg / c->p.box) : alpha;
   const int3 nr = make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m));

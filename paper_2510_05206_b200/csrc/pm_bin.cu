@@ -6,7 +6,7 @@
 //   scan    k_scan_*  : exclusive scans of the tile counts and of the per-tile work-item counts
 //   pass 2  k_permute : recompute the coordinate, claim a slot (warp-aggregated, order-preserving inside a
 //                       warp), store the record {ux, uy, uz, i} with tile-local fixed-point coordinates
-//   items   k_items   : work items (tile, begin, end) of at most CHUNK particles
+//   items   k_items   : work items (tile, begin, end) of at most ITEM_MAX particles (even split of dense tiles)
 //
 // Algorithmic bytes: 12N (read) + 12N (read) + 16N (write); the tile arrays are O(ntiles).
 #include "pm_internal.cuh"
@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
 // ---- exclusive scan of (count, nchunks) over the tiles: reduce / scan-of-partials / rescan ----------
 constexpr int SCAN_T = 1024, SCAN_E = 4, SCAN_B = SCAN_T * SCAN_E;
 
-__device__ __forceinline__ uint32_t nchunks_of(uint32_t cnt) { return (cnt + CHUNK - 1) / CHUNK; }
+__device__ __forceinline__ uint32_t nchunks_of(uint32_t cnt) { return (cnt + ITEM_MAX - 1) / ITEM_MAX; }
 
 __device__ uint2 block_exclusive_scan(uint2 v, uint2* total) {  // blockDim.x == SCAN_T
   __shared__ uint2 wsum[32];
@@ -295,11 +295,13 @@ __global__ void __launch_bounds__(256) k_items(const uint32_t* __restrict__ tile
   r >>= xbl;
   const int ty = r % nty, tx = ((r / nty) << xbl) | xl;
   const uint32_t txyz = (uint32_t)tx | ((uint32_t)ty << 10) | ((uint32_t)tz << 20);
-  for (uint32_t s = b; s < e; s += CHUNK) {
+  const uint32_t k = nchunks_of(e - b);
+  const uint32_t per = k ? (e - b + k - 1) / k : 0;  // even split: no tiny remainder items
+  for (uint32_t j = 0; j < k; ++j) {  // exactly the k slots the scan reserved (a slot may stay empty)
     WorkItem w;
     w.tile = (uint32_t)t;
-    w.begin = s;
-    w.end = min(s + (uint32_t)CHUNK, e);
+    w.begin = min(b + j * per, e);
+    w.end = min(w.begin + per, e);
     w.txyz = txyz;
     items[it++] = w;
   }

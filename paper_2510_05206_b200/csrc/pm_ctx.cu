@@ -243,7 +243,7 @@ static int build(Ctx* c) {
 
   // binning workspace
   c->cap = p.max_particles;
-  c->max_items = (int64_t)c->ntiles + c->cap / CHUNK + 2;
+  c->max_items = (int64_t)c->ntiles + c->cap / ITEM_MAX + 2;
   const int scan_blocks = (c->ntiles + 4095) / 4096;
   PM_CUDA(c, cudaMalloc((void**)&c->rec, sizeof(uint4) * (size_t)c->cap));
   PM_CUDA(c, cudaMalloc((void**)&c->tile_cnt, sizeof(uint32_t) * (size_t)c->ntiles));

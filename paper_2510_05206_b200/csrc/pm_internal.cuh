@@ -6,7 +6,7 @@
 //     coordinates in unsigned fixed point, value = (u_local + REC_BIAS) * 2^REC_FRAC, computed once in
 //     fp64 by the binning pass (the fp32 product x*(m/L) alone would cost 1e-5 of force accuracy).
 //   * tiles of TX x TY x TZ cells in z-fastest order; tile_off[ntiles+1]; work items (tile, begin, end)
-//     of at most CHUNK particles.
+//     of at most ITEM_MAX particles.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -24,7 +24,9 @@ constexpr int TX = 8, TY = 8, TZ = 32;  // cells per tile: a warp's 32 consecuti
                                         // one z row, so their shared-memory accesses fall in 32 different banks
 constexpr int BLOCK = 256;              // threads per CTA of the scatter / gather kernels
 constexpr int PPT = 8;                  // particles per thread and work item
-constexpr int CHUNK = BLOCK * PPT;      // max particles per work item
+constexpr int CHUNK = BLOCK * PPT;      // particles a CTA holds in registers at a time
+constexpr int ITEM_MAX = 2 * CHUNK;     // max particles per work item: a tile is one item unless it is denser than
+                                        // this (clustered inputs), then it is split evenly for load balance
 constexpr int REC_FRAC = 26;            // fractional bits of a record coordinate
 constexpr int REC_BIAS = 2;             // cells added so that shifted / half-added values stay >= 0
 constexpr uint32_t REC_ONE = 1u << REC_FRAC;

@@ -1,7 +1,7 @@
 // pm_mesh_kernels.cuh -- the tile scatter (K2/K5) and tile gather (K4/K7) kernels, templated on the
 // interpolation kernel ("Traits": B-splines of Table 1, or the exponential-of-semicircle kernel).
 //
-// One work item = one mesh tile (TX x TY x TZ cells) and at most CHUNK of its sorted particles.
+// One work item = one mesh tile (TX x TY x TZ cells) and at most ITEM_MAX of its sorted particles.
 //   scatter: the tile plus its halo is accumulated in shared memory with native 32-bit integer atomics
 //            (sm_100a has no native fp32 shared atomic: atomicAdd(float*) on shared memory compiles to a
 //            CAS loop, 2.5x slower measured).  The fixed-point scale is chosen per work item from
@@ -264,13 +264,16 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
   // loop, so their latency is covered by the flush of the current tile.
   WorkItem wi;
   uint4 r[PPT];
-  auto load_item = [&](uint32_t id) {
-    wi = bv.items[id];
+  auto load_batch = [&](uint32_t b0, uint32_t end) {  // up to CHUNK records starting at b0
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
-      const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
-      if (i < wi.end) r[k] = load_rec(bv.rec + i);
+      const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
+      if (i < end) r[k] = load_rec(bv.rec + i);
     }
+  };
+  auto load_item = [&](uint32_t id) {
+    wi = bv.items[id];
+    load_batch(wi.begin, wi.end);
   };
   uint32_t it = blockIdx.x;
   int par = 0;
@@ -285,15 +288,25 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
     float wabs[NCOMP];
 #pragma unroll
     for (int a = 0; a < NCOMP; ++a) wabs[a] = 0.0f;
+    auto load_weights = [&](uint32_t b0) {  // weights of the batch held in r[]
 #pragma unroll
-    for (int k = 0; k < PPT; ++k) {
-      const uint32_t i = ibegin + (uint32_t)(k * BLOCK + tid);
-      if (i < iend) {
+      for (int k = 0; k < PPT; ++k) {
+        const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
+        if (i < iend) {
 #pragma unroll
-        for (int a = 0; a < NCOMP; ++a) {
-          wv[k][a] = WEIGHTED ? __ldg(wsrc + (size_t)r[k].w * wstride + a) : 1.0f;
-          wabs[a] += fabsf(wv[k][a]);
+          for (int a = 0; a < NCOMP; ++a) {
+            wv[k][a] = WEIGHTED ? __ldg(wsrc + (size_t)r[k].w * wstride + a) : 1.0f;
+            wabs[a] += fabsf(wv[k][a]);
+          }
         }
+      }
+    };
+    load_weights(ibegin);
+    if (WEIGHTED && n > (uint32_t)CHUNK) {  // dense tile: the bound needs the weights of the later batches too
+      for (uint32_t i = ibegin + CHUNK + tid; i < iend; i += BLOCK) {
+        const uint32_t idx = bv.rec[i].w;
+#pragma unroll
+        for (int a = 0; a < NCOMP; ++a) wabs[a] += fabsf(__ldg(wsrc + (size_t)idx * wstride + a));
       }
     }
 
@@ -336,9 +349,10 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
       }
     }
 
+    for (uint32_t b0 = ibegin;;) {
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
-      const uint32_t i = ibegin + (uint32_t)(k * BLOCK + tid);
+      const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
       if (i < iend) {
         int sx, sy, sz;
         float wx[P], wy[P], wz[P], dummy[P];
@@ -371,6 +385,11 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
             }
           }
       }
+    }
+      b0 += CHUNK;
+      if (b0 >= iend) break;  // uniform
+      load_batch(b0, iend);   // dense tile: further batches of the same item
+      load_weights(b0);
     }
     __syncthreads();
     it = s_next[par];
@@ -671,7 +690,7 @@ inline int norm_roll(int r, int m) {
 
 // Grid of a persistent mesh kernel: resident CTAs per SM x SMs, capped by an upper bound of the item count.
 inline int mesh_grid(const Ctx* c, int occ) {
-  int64_t bound = (int64_t)c->ntiles + c->bin_n / CHUNK + 1;
+  int64_t bound = (int64_t)c->ntiles + c->bin_n / ITEM_MAX + 1;
   int64_t cap = (int64_t)c->num_sms * (occ < 1 ? 1 : occ);
   return (int)(bound < cap ? bound : cap);
 }

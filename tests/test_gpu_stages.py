@@ -125,7 +125,10 @@ def test_interp_vjp_parity(pm, worder, ncomp):
     pm.pm_interp_vjp(ctx, [dev(meshes[a]) for a in range(ncomp)], dev(pos), dev(cot), mesh_cot=mesh_cot, pos_cot=pos_cot)
     for a in range(ncomp):
         ref = po.scatter(pos, M, BOX, worder, weights=cot[:, a])
-        assert rel_l2(mesh_cot[a].cpu().numpy(), ref) <= 3e-6  # random-sign weights in a dense clump
+        # random-sign weights in a dense clump: the node sums cancel, while the fixed-point quantum is 2^-30 of the
+        # work item's bound sum|w| * Wmax^3 ("Parity bars"); with items of up to 4096 particles that is
+        # the accuracy of an fp32 accumulation in the same order, not better
+        assert rel_l2(mesh_cot[a].cpu().numpy(), ref) <= 5e-6
     ref_p = np.zeros((n, 3))
     for a in range(ncomp):
         for b in range(3):

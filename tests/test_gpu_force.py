@@ -238,3 +238,25 @@ def test_pm_force_host_matches_device(pm):
     ms, launches = pm.pm_get_stage_ms(ctx)
     assert launches >= 8 and ms["assign"] > 0 and ms["interp"] > 0
     pm.pm_destroy(ctx)
+
+
+def test_force_parity_headline_full_size_sampled(pm):
+    """The bench workload itself (N = 512^3 particles, 512^3 mesh, the launch configuration bench.py times):
+    the oracle assigns all particles and solves for the three force meshes at full size in fp64, then
+    interpolates them for a seeded sample of particles, one by one; plus the invariant that holds at any size,
+    momentum conservation sum_i F_i = 0 (interlace 0)."""
+    pos, c = gen.make_config_positions("headline")
+    n = pos.shape[0]
+    f = gpu_force(pm, params_of(pm, c, n), pos)
+    kw = oracle_kw(c)
+    kw.pop("interlace")
+    d = po.density_contrast(po.scatter(pos, c["m"], c["box"], kw["worder"]), n)
+    g = po.poisson_force(d, box=c["box"], **kw)
+    del d
+    idx = np.sort(np.random.default_rng(4242).choice(n, size=200_000, replace=False))
+    ref = np.stack([po.gather(g[a], pos[idx], c["box"], kw["worder"]) for a in range(3)], axis=1)
+    err = rel_l2(f[idx], ref)
+    record_error("force/headline/n_p=512/sampled=200000", err, FORCE_TOL)
+    assert err <= FORCE_TOL
+    fsum = np.abs(f.astype(np.float64).sum(axis=0)).max()
+    assert fsum <= 1e-6 * np.abs(f.astype(np.float64)).sum()

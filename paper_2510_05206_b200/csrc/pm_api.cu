@@ -30,16 +30,7 @@ int ensure_vjp_buffers(Ctx* c) {
 // delta spectra of the ctx meshes rho[0] (, rho[1]) -> force meshes g[0..2].  coeff_eff carries every
 // scalar: coeff, the density-contrast factor m^3/N of Eq. 2.3 and cuFFT's missing 1/m^3.
 int spectra_to_force_meshes(Ctx* c, int ngrids, double coeff_eff, cudaStream_t st) {
-  stage_begin(c, PM_STAGE_FFT_FWD, st);
-  for (int i = 0; i < ngrids; ++i) PM_TRY(fft_r2c(c, c->rho[i], c->dhat[i], st));
-  stage_end(c, PM_STAGE_FFT_FWD, st);
-  stage_begin(c, PM_STAGE_KSPACE, st);
-  PM_TRY(launch_kspace_forward(c, c->dhat[0], ngrids == 2 ? c->dhat[1] : nullptr, c->ghat, coeff_eff, st));
-  stage_end(c, PM_STAGE_KSPACE, st);
-  stage_begin(c, PM_STAGE_FFT_INV, st);
-  for (int a = 0; a < 3; ++a) PM_TRY(fft_c2r(c, c->ghat[a], c->g[a], st));
-  stage_end(c, PM_STAGE_FFT_INV, st);
-  return PM_OK;
+  return spectral_forward(c, c->rho[0], ngrids == 2 ? c->rho[1] : nullptr, c->g, coeff_eff, true, st);
 }
 
 // a1: assignment of unit-mass particles onto the ctx meshes (interlace 1: also the half-cell shifted grid)
@@ -93,10 +84,7 @@ int force_vjp_single(Ctx* c, int64_t N, const ShiftSplit& sh, bool second_grid, 
   stage_end(c, PM_STAGE_VJP_SCATTER, st);
   // (iii) rho_bar = IFFT( sum_a conj(S_a) FFT(gbar_a) ), with the m^3/N of the density contrast folded in
   stage_begin(c, PM_STAGE_VJP_KSPACE, st);
-  for (int a = 0; a < 3; ++a) PM_TRY(fft_r2c(c, c->gbar[a], c->ghat[a], st));
-  PM_TRY(launch_kspace_transpose(c, c->ghat, c->dhat[0], second_grid ? c->dhat[1] : nullptr, coeff_eff, st));
-  PM_TRY(fft_c2r(c, c->dhat[0], c->rho[0], st));
-  if (second_grid) PM_TRY(fft_c2r(c, c->dhat[1], c->rho[1], st));
+  PM_TRY(spectral_transpose(c, c->gbar, c->rho[0], second_grid ? c->rho[1] : nullptr, coeff_eff, st));
   stage_end(c, PM_STAGE_VJP_KSPACE, st);
   // (i) + (iv): grad-W gathers (Eq. C.12 weighted by lam, Eq. C.6 with w_i = 1)
   stage_begin(c, PM_STAGE_VJP_GATHER, st);
@@ -163,11 +151,7 @@ int pm_poisson_force(pm_ctx* ctx, const float* delta_mesh, const float* delta_me
   if (two != (delta_mesh2 != nullptr))
     return fail(c, PM_EINVAL, "delta_mesh2 must be given iff interlace = 1");
   cudaStream_t st = S(stream);
-  PM_TRY(fft_r2c(c, delta_mesh, c->dhat[0], st));
-  if (two) PM_TRY(fft_r2c(c, delta_mesh2, c->dhat[1], st));
-  PM_TRY(launch_kspace_forward(c, c->dhat[0], two ? c->dhat[1] : nullptr, c->ghat, c->p.coeff / (double)c->G, st));
-  for (int a = 0; a < 3; ++a) PM_TRY(fft_c2r(c, c->ghat[a], force_mesh[a], st));
-  return PM_OK;
+  return spectral_forward(c, delta_mesh, two ? delta_mesh2 : nullptr, force_mesh, c->p.coeff / (double)c->G, false, st);
 }
 
 int pm_poisson_force_vjp(pm_ctx* ctx, const float* const force_cot[3], float* delta_cot, float* delta_cot2,
@@ -180,11 +164,7 @@ int pm_poisson_force_vjp(pm_ctx* ctx, const float* const force_cot[3], float* de
   if (two != (delta_cot2 != nullptr))
     return fail(c, PM_EINVAL, "delta_cot2 must be given iff interlace = 1");
   cudaStream_t st = S(stream);
-  for (int a = 0; a < 3; ++a) PM_TRY(fft_r2c(c, force_cot[a], c->ghat[a], st));
-  PM_TRY(launch_kspace_transpose(c, c->ghat, c->dhat[0], two ? c->dhat[1] : nullptr, c->p.coeff / (double)c->G, st));
-  PM_TRY(fft_c2r(c, c->dhat[0], delta_cot, st));
-  if (two) PM_TRY(fft_c2r(c, c->dhat[1], delta_cot2, st));
-  return PM_OK;
+  return spectral_transpose(c, force_cot, delta_cot, two ? delta_cot2 : nullptr, c->p.coeff / (double)c->G, st);
 }
 
 int pm_interp(pm_ctx* ctx, const float* const mesh[], int ncomp, const float* pos, int64_t N, const double* shift,
@@ -245,10 +225,7 @@ int nufft_poisson_force(pm_ctx* ctx, const float* fine, int64_t n_particles, flo
   if (!fine || !force_fine || !force_fine[0] || !force_fine[1] || !force_fine[2] || n_particles < 1)
     return fail(c, PM_EINVAL, "NULL mesh pointer or n_particles < 1");
   cudaStream_t st = S(stream);
-  PM_TRY(fft_r2c(c, fine, c->dhat[0], st));
-  PM_TRY(launch_kspace_forward(c, c->dhat[0], nullptr, c->ghat, c->p.coeff / (double)n_particles, st));
-  for (int a = 0; a < 3; ++a) PM_TRY(fft_c2r(c, c->ghat[a], force_fine[a], st));
-  return PM_OK;
+  return spectral_forward(c, fine, nullptr, force_fine, c->p.coeff / (double)n_particles, false, st);
 }
 
 int nufft_poisson_force_vjp(pm_ctx* ctx, const float* const force_cot[3], int64_t n_particles, float* fine_cot,
@@ -258,9 +235,7 @@ int nufft_poisson_force_vjp(pm_ctx* ctx, const float* const force_cot[3], int64_
   if (!fine_cot || !force_cot || !force_cot[0] || !force_cot[1] || !force_cot[2] || n_particles < 1)
     return fail(c, PM_EINVAL, "NULL mesh pointer or n_particles < 1");
   cudaStream_t st = S(stream);
-  for (int a = 0; a < 3; ++a) PM_TRY(fft_r2c(c, force_cot[a], c->ghat[a], st));
-  PM_TRY(launch_kspace_transpose(c, c->ghat, c->dhat[0], nullptr, c->p.coeff / (double)n_particles, st));
-  return fft_c2r(c, c->dhat[0], fine_cot, st);
+  return spectral_transpose(c, force_cot, fine_cot, nullptr, c->p.coeff / (double)n_particles, st);
 }
 
 int nufft_interp(pm_ctx* ctx, const float* const fine[], int ncomp, const float* pos, int64_t N, float* out,

@@ -266,10 +266,16 @@ static int build(Ctx* c) {
   PM_CUFFT(c, cufftMakePlan3d(c->plan_r2c, mg, mg, mg, CUFFT_R2C, &ws1));
   PM_CUFFT(c, cufftMakePlan3d(c->plan_c2r, mg, mg, mg, CUFFT_C2R, &ws2));
   c->fft_work_bytes = ws1 > ws2 ? ws1 : ws2;
-  if (c->fft_work_bytes) {
+  PM_TRY(xfft_init(c));  // 2-D plans + twiddles of the fused x-FFT path, when m allows it
+  if (c->xfused && c->fft2_work_bytes > c->fft_work_bytes) c->fft_work_bytes = c->fft2_work_bytes;
+  if (c->fft_work_bytes) {  // one work area: the plans never run concurrently (one stream per ctx)
     PM_CUDA(c, cudaMalloc(&c->fft_work, c->fft_work_bytes));
     PM_CUFFT(c, cufftSetWorkArea(c->plan_r2c, c->fft_work));
     PM_CUFFT(c, cufftSetWorkArea(c->plan_c2r, c->fft_work));
+    if (c->xfused) {
+      PM_CUFFT(c, cufftSetWorkArea(c->plan2_r2c, c->fft_work));
+      PM_CUFFT(c, cufftSetWorkArea(c->plan2_c2r, c->fft_work));
+    }
   }
 
   // meshes of the fused path
@@ -295,10 +301,14 @@ static void teardown(Ctx* c) {
     cufftDestroy(c->plan_r2c);
     cufftDestroy(c->plan_c2r);
   }
+  if (c->plans2_ok) {
+    cufftDestroy(c->plan2_r2c);
+    cufftDestroy(c->plan2_c2r);
+  }
   void* ptrs[] = {c->tab_grad, c->tab_lap, c->tab_win, c->tab_cos, c->tab_sin, c->rec, c->tile_cnt,
                   c->tile_off, c->item_off, c->scan_tmp, c->items, c->nitems, c->sched, c->fft_work, c->rho[0],
                   c->rho[1], c->dhat[0], c->dhat[1], c->ghat[0], c->ghat[1], c->ghat[2], c->g[0],
-                  c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->host_pos_dev,
+                  c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->xtw, c->host_pos_dev,
                   c->host_force_dev};
   for (void* q : ptrs)
     if (q) cudaFree(q);

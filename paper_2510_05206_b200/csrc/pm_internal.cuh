@@ -124,6 +124,12 @@ struct Ctx {
   bool plans_ok;
   void* fft_work;
   size_t fft_work_bytes;
+  // fused x-FFT + k-space path (pm_xfft.cu): batched 2-D (y,z) plans, twiddles e^{-2 pi i k/m}
+  bool xfused;
+  bool plans2_ok;
+  cufftHandle plan2_r2c, plan2_c2r;
+  size_t fft2_work_bytes;
+  float2* xtw;
 
   // meshes owned by the ctx (pm_force path)
   float* rho[2];     // assignment targets (second: interlace = 1)
@@ -204,6 +210,20 @@ int launch_kspace_transpose(Ctx* c, const float2* const gh[3], float2* q1, float
                             double coeff_eff, cudaStream_t st);
 int fft_r2c(Ctx* c, const float* in, float2* out, cudaStream_t st);
 int fft_c2r(Ctx* c, float2* in, float* out, cudaStream_t st);
+// fused path: 2-D (y,z) transforms by cuFFT, x transforms + k-space kernel in one kernel (pm_xfft.cu)
+int xfft_init(Ctx* c);
+int fft2_r2c(Ctx* c, const float* in, float2* out, cudaStream_t st);
+int fft2_c2r(Ctx* c, float2* in, float* out, cudaStream_t st);
+int launch_xfft_forward(Ctx* c, const float2* d1, const float2* d2, float2* const gh[3], double coeff_eff,
+                        cudaStream_t st);
+int launch_xfft_transpose(Ctx* c, const float2* const gh[3], float2* q1, float2* q2, double coeff_eff,
+                          cudaStream_t st);
+// The whole spectral operator on real meshes (a2-a4 resp. a10), fused when the ctx supports it:
+//   forward:   delta (, delta2) -> g[0..2];     transpose: gbar[0..2] -> delta_cot (, delta_cot2)
+// dhat / ghat of the ctx are the scratch spectra.  stages = true records the bench's stage events.
+int spectral_forward(Ctx* c, const float* d1, const float* d2, float* const g[3], double coeff_eff, bool stages,
+                     cudaStream_t st);
+int spectral_transpose(Ctx* c, const float* const gb[3], float* q1, float* q2, double coeff_eff, cudaStream_t st);
 
 // profiling helpers
 void stage_begin(Ctx* c, int stage, cudaStream_t st);

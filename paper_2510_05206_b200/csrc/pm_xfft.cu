@@ -1,0 +1,446 @@
+// pm_xfft.cu -- a2-a4 / a7 / a10 fused along x: the x-direction passes of the forward and inverse 3-D FFTs and the
+// Fourier-space kernel (K3, K6, and its transpose) in ONE kernel.
+//
+// The 3-D transforms are split as (y,z) planes x lines.  cuFFT does the batched 2-D (y,z) transforms (library
+// call, "FFT"); this kernel then takes, for 8 neighbouring (y,z) columns at a time, the whole x line
+// into shared memory, runs the forward x-FFT, applies the Green's function / gradient symbols / deconvolution /
+// interlace combine of pm_kspace.cu (Tables 1-2) and runs the three inverse x-FFTs, so that
+// the spectrum is read once and the three force spectra are written once.  Unfused, the same work is five more
+// passes over the data: forward x pass (read + write), k-space kernel (read, 3 writes), three inverse x passes
+// (read + write each): 6.4 GB instead of 2.1 GB at 512^3.
+//
+// FFT: in-place mixed-radix (8 / 16) Cooley-Tukey in shared memory.  Forward = decimation in frequency (natural
+// order in, digit-reversed out), inverse = decimation in time with the stages in reverse order (digit-reversed in,
+// natural out), so no reordering pass is needed: the pointwise kernel maps a position to its frequency.
+// Unnormalised both ways, like cuFFT; the 1/m^3 is folded into coeff_eff by the caller.
+// Built for m = 64 ... 1024, powers of two; other sizes take the unfused path (cuFFT 3-D + pm_kspace.cu).
+#include <math.h>
+
+#include <vector>
+
+#include "pm_internal.cuh"
+
+namespace pmf {
+
+constexpr int XC = 8;    // (y,z) columns per CTA: 64 contiguous bytes of every x plane
+constexpr int XEPT = 16; // elements per thread -> N * XC / 16 threads per CTA
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmulx(float2 a, float2 b) {
+  return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) {  // a * conj(b)
+  return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+// multiply by SIGN * i  (SIGN = -1: forward transform, e^{-2 pi i/4} = -i; SIGN = +1: inverse)
+template <int SIGN>
+__device__ __forceinline__ float2 mul_i(float2 a) {
+  return SIGN < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+}
+
+// ---- small DFTs in registers, X_k = sum_n x_n e^{SIGN 2 pi i n k / R}, natural order in and out ---------
+template <int SIGN>
+__device__ __forceinline__ void dft4(float2& a0, float2& a1, float2& a2, float2& a3) {
+  const float2 t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = mul_i<SIGN>(csub(a1, a3));
+  a0 = cadd(t0, t2);
+  a2 = csub(t0, t2);
+  a1 = cadd(t1, t3);
+  a3 = csub(t1, t3);
+}
+
+template <int R, int SIGN>
+struct Dft;
+
+template <int SIGN>
+struct Dft<8, SIGN> {
+  static __device__ __forceinline__ void run(float2 (&v)[8]) {
+    // even / odd samples: X_k = E_k + W8^k O_k, X_{k+4} = E_k - W8^k O_k
+    dft4<SIGN>(v[0], v[2], v[4], v[6]);
+    dft4<SIGN>(v[1], v[3], v[5], v[7]);
+    constexpr float h = 0.70710678118654752f;
+    // W8^k = e^{SIGN 2 pi i k / 8}
+    const float2 o0 = v[1];
+    const float2 o1 = make_float2(h * (v[3].x - SIGN * v[3].y), h * (v[3].y + SIGN * v[3].x));   // * (1 + SIGN i)/sqrt2
+    const float2 o2 = mul_i<SIGN>(v[5]);
+    const float2 o3 = make_float2(h * (-v[7].x - SIGN * v[7].y), h * (-v[7].y + SIGN * v[7].x)); // * (-1 + SIGN i)/sqrt2
+    const float2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6];
+    v[0] = cadd(e0, o0);
+    v[4] = csub(e0, o0);
+    v[1] = cadd(e1, o1);
+    v[5] = csub(e1, o1);
+    v[2] = cadd(e2, o2);
+    v[6] = csub(e2, o2);
+    v[3] = cadd(e3, o3);
+    v[7] = csub(e3, o3);
+  }
+};
+
+template <int SIGN>
+struct Dft<16, SIGN> {
+  static __device__ __forceinline__ void run(float2 (&v)[16]) {
+    // n = 4 n' + s: A_s = DFT4(x_s, x_{s+4}, x_{s+8}, x_{s+12}); X_{k+4q} = sum_s W4^{sq} (W16^{sk} A_s[k])
+#pragma unroll
+    for (int s = 0; s < 4; ++s) dft4<SIGN>(v[s], v[s + 4], v[s + 8], v[s + 12]);  // A_s[k] now in v[s + 4k]
+    constexpr float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
+    // W16^j = cos(pi j / 8) + SIGN i sin(pi j / 8), j = s k in {1, 2, 3, 4, 6, 9}
+    const float2 w1 = make_float2(c1, SIGN * s1), w2 = make_float2(h, SIGN * h), w3 = make_float2(s1, SIGN * c1);
+    const float2 w6 = make_float2(-h, SIGN * h), w9 = make_float2(-c1, -SIGN * s1);
+    v[1 + 4] = cmulx(v[1 + 4], w1);    // s = 1, k = 1
+    v[1 + 8] = cmulx(v[1 + 8], w2);    // s = 1, k = 2
+    v[1 + 12] = cmulx(v[1 + 12], w3);  // s = 1, k = 3
+    v[2 + 4] = cmulx(v[2 + 4], w2);    // s = 2, k = 1
+    v[2 + 8] = mul_i<SIGN>(v[2 + 8]);  // s = 2, k = 2: W16^4 = SIGN i
+    v[2 + 12] = cmulx(v[2 + 12], w6);  // s = 2, k = 3
+    v[3 + 4] = cmulx(v[3 + 4], w3);    // s = 3, k = 1
+    v[3 + 8] = cmulx(v[3 + 8], w6);    // s = 3, k = 2
+    v[3 + 12] = cmulx(v[3 + 12], w9);  // s = 3, k = 3
+#pragma unroll
+    for (int k = 0; k < 4; ++k) dft4<SIGN>(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);  // over s -> q
+    // v[4k + q] = X_{k + 4q}: transpose to natural order
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+      for (int q = k + 1; q < 4; ++q) {
+        const float2 t = v[4 * k + q];
+        v[4 * k + q] = v[4 * q + k];
+        v[4 * q + k] = t;
+      }
+  }
+};
+
+// ---- shared-memory line layout and the FFT stages -----------------------------------------------------------
+// Element (x position p, column c) sits at float2 index p * XC + c + 8 * (p / 8): a row of 8 columns is half of
+// the 32 banks; the padding puts rows p and p + 8 (last stage) in different halves, rows p and p + 1 are anyway.
+__device__ __forceinline__ int sidx(int p, int c) { return p * XC + c + ((p >> 3) << 3); }
+template <int N>
+constexpr int xfft_smem_elems() { return N * XC + (N / 8) * 8; }
+
+template <int N>
+struct Radices;  // N = r0 * r1 * r2
+template <> struct Radices<64>   { static constexpr int r0 = 8,  r1 = 8,  r2 = 1; };
+template <> struct Radices<128>  { static constexpr int r0 = 16, r1 = 8,  r2 = 1; };
+template <> struct Radices<256>  { static constexpr int r0 = 16, r1 = 16, r2 = 1; };
+template <> struct Radices<512>  { static constexpr int r0 = 8,  r1 = 8,  r2 = 8; };
+template <> struct Radices<1024> { static constexpr int r0 = 16, r1 = 8,  r2 = 8; };
+
+// One radix-R stage over sub-transforms of size S (M = S / R butterflies each).  tw[k] = e^{-2 pi i k / N}.
+//   forward (DIF): y = DFT_R(x), y_q *= W_S^{jq};      inverse (DIT): x_r *= conj(W_S)^{jr}, y = IDFT_R(x)
+template <int N, int R, int S, bool INV>
+__device__ __forceinline__ void xfft_stage(float2* s, const float2* tw, int tid) {
+  constexpr int M = S / R, NB = N * XC / R, NT = N * XC / XEPT;
+#pragma unroll
+  for (int b = tid; b < NB; b += NT) {
+    const int c = b % XC, bf = b / XC, blk = bf / M, j = bf % M;
+    const int p0 = blk * S + j;
+    float2 v[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) v[r] = s[sidx(p0 + r * M, c)];
+    if (INV) {
+#pragma unroll
+      for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], __ldg(tw + (N / S) * j * r));
+      Dft<R, 1>::run(v);
+    } else {
+      Dft<R, -1>::run(v);
+#pragma unroll
+      for (int q = 1; q < R; ++q) v[q] = cmulx(v[q], __ldg(tw + (N / S) * j * q));
+    }
+#pragma unroll
+    for (int q = 0; q < R; ++q) s[sidx(p0 + q * M, c)] = v[q];
+  }
+  __syncthreads();
+}
+
+template <int N, bool INV>
+__device__ __forceinline__ void xfft_line(float2* s, const float2* tw, int tid) {
+  using Rd = Radices<N>;
+  constexpr int S1 = N / Rd::r0, S2 = S1 / Rd::r1;
+  if (!INV) {
+    xfft_stage<N, Rd::r0, N, false>(s, tw, tid);
+    xfft_stage<N, Rd::r1, S1, false>(s, tw, tid);
+    if (Rd::r2 > 1) xfft_stage<N, (Rd::r2 > 1 ? Rd::r2 : 8), (Rd::r2 > 1 ? S2 : 8), false>(s, tw, tid);
+  } else {
+    if (Rd::r2 > 1) xfft_stage<N, (Rd::r2 > 1 ? Rd::r2 : 8), (Rd::r2 > 1 ? S2 : 8), true>(s, tw, tid);
+    xfft_stage<N, Rd::r1, S1, true>(s, tw, tid);
+    xfft_stage<N, Rd::r0, N, true>(s, tw, tid);
+  }
+}
+
+// frequency index held at position p after the forward (DIF) stages: p = q0 * (N/r0) + q1 * (N/(r0 r1)) + q2,
+// k = q0 + r0 * (q1 + r1 * q2)
+template <int N>
+__device__ __forceinline__ int xfft_freq(int p) {
+  using Rd = Radices<N>;
+  constexpr int S1 = N / Rd::r0, S2 = S1 / Rd::r1;
+  const int q0 = p / S1, rem = p - q0 * S1, q1 = rem / S2, q2 = rem - q1 * S2;
+  return q0 + Rd::r0 * (q1 + Rd::r1 * q2);
+}
+
+struct XTabs {
+  const double *grad, *lap, *win, *pc, *ps;  // per-axis symbol tables of pm_kspace.cu
+  const float2* tw;                          // e^{-2 pi i k / m}, k = 0 .. m-1
+  int m, hz;
+  int64_t ncol;                              // m * hz columns per x plane
+};
+
+// One CTA: XC consecutive columns q = iy * hz + iz of the (y,z) plane, all m values of x.
+//   MODE 0 (force):     in0 (, in1 = second interlaced grid) -> out0..2 = x-inverse of S_a(n) dhat(n)
+//   MODE 1 (transpose): in0..2 -> out0 (, out1) = x-inverse of sum_a conj(S_a) ghat_a
+// Every input is the (y,z)-transformed, x-untransformed spectrum [x][y][hz]; every output likewise.
+template <int N, int MODE>
+__global__ void __launch_bounds__(N* XC / XEPT) k_xfft_kspace(XTabs t, const float2* __restrict__ in0,
+                                                               const float2* __restrict__ in1,
+                                                               const float2* __restrict__ in2,
+                                                               float2* __restrict__ out0, float2* __restrict__ out1,
+                                                               float2* __restrict__ out2, double coeff_eff) {
+  constexpr int NT = N * XC / XEPT;
+  constexpr int SE = xfft_smem_elems<N>();
+  extern __shared__ __align__(16) float2 s_x[];
+  float2* s_w = s_x;        // work line: FFT in place
+  float2* s_a = s_x + SE;   // MODE 0: green * dhat;  MODE 1: accumulated q
+  const float2* s_tw = t.tw;  // 8 m bytes, read through L1 (keeps three 512-point CTAs per SM)
+  const int tid = threadIdx.x;
+  const int c = tid % XC;   // this thread's column in every pointwise loop (NT is a multiple of XC)
+  const int64_t q = (int64_t)blockIdx.x * XC + c;
+  const bool live = q < t.ncol;
+  const int iy = live ? (int)(q / t.hz) : 0, iz = live ? (int)(q - (int64_t)iy * t.hz) : 0;
+  const size_t plane = (size_t)t.ncol;
+
+  auto load_line = [&](const float2* __restrict__ src) {
+    float2 v[XEPT];
+#pragma unroll
+    for (int i = 0; i < XEPT; ++i) {
+      const int p = tid / XC + i * (NT / XC);
+      v[i] = live ? __ldcs(src + (size_t)p * plane + q) : make_float2(0.f, 0.f);
+    }
+#pragma unroll
+    for (int i = 0; i < XEPT; ++i) s_w[sidx(tid / XC + i * (NT / XC), c)] = v[i];
+    __syncthreads();
+  };
+  auto store_line = [&](float2* __restrict__ dst) {  // after the inverse stages (they end with a barrier)
+#pragma unroll
+    for (int i = 0; i < XEPT; ++i) {
+      const int p = tid / XC + i * (NT / XC);
+      if (live) dst[(size_t)p * plane + q] = s_w[sidx(p, c)];
+    }
+    __syncthreads();
+  };
+
+  // column factors
+  const double lyz = t.lap[iy] + t.lap[iz], wyz = t.win[iy] * t.win[iz];
+  const float dyv = (float)t.grad[iy], dzv = (float)t.grad[iz];
+  const double pcyz = t.pc[iy] * t.pc[iz] - t.ps[iy] * t.ps[iz], psyz = t.pc[iy] * t.ps[iz] + t.ps[iy] * t.pc[iz];
+
+  auto green_of = [&](int kx) -> double {  // coeff / (Lap * window); 0 at n = 0 and for dropped modes
+    const double den = (lyz + t.lap[kx]) * (wyz * t.win[kx]);
+    return den != 0.0 ? coeff_eff / den : 0.0;
+  };
+  auto phase_of = [&](int kx) -> float2 {  // interlace phase e^{-ik.s} (real part only on Nyquist planes, R9)
+    return make_float2((float)(t.pc[kx] * pcyz - t.ps[kx] * psyz), (float)(t.pc[kx] * psyz + t.ps[kx] * pcyz));
+  };
+
+  if (MODE == 0) {
+    const bool two = in1 != nullptr;
+    if (two) {  // second grid first: s_a = 1/2 phase * dhat2
+      load_line(in1);
+      xfft_line<N, false>(s_w, s_tw, tid);
+#pragma unroll
+      for (int i = 0; i < XEPT; ++i) {
+        const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
+        const float2 e = cmulx(phase_of(kx), s_w[sidx(p, c)]);
+        s_a[sidx(p, c)] = make_float2(0.5f * e.x, 0.5f * e.y);
+      }
+      __syncthreads();
+    }
+    load_line(in0);
+    xfft_line<N, false>(s_w, s_tw, tid);
+#pragma unroll
+    for (int i = 0; i < XEPT; ++i) {  // s_a = green * dhat (each thread touches only its own elements of s_a)
+      const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
+      float2 d = s_w[sidx(p, c)];
+      if (two) {
+        const float2 e = s_a[sidx(p, c)];
+        d = make_float2(0.5f * d.x + e.x, 0.5f * d.y + e.y);
+      }
+      const float g = (float)green_of(kx);
+      s_a[sidx(p, c)] = make_float2(g * d.x, g * d.y);
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int a = 0; a < 3; ++a) {
+#pragma unroll
+      for (int i = 0; i < XEPT; ++i) {  // -i D_a (re + i im) = D_a (im - i re)
+        const int p = tid / XC + i * (NT / XC);
+        const float dm = a == 0 ? (float)t.grad[xfft_freq<N>(p)] : (a == 1 ? dyv : dzv);
+        const float2 d = s_a[sidx(p, c)];
+        s_w[sidx(p, c)] = make_float2(dm * d.y, -dm * d.x);
+      }
+      __syncthreads();
+      xfft_line<N, true>(s_w, s_tw, tid);
+      store_line(a == 0 ? out0 : (a == 1 ? out1 : out2));
+    }
+  } else {
+    const bool two = out1 != nullptr;
+#pragma unroll 1
+    for (int a = 0; a < 3; ++a) {
+      load_line(a == 0 ? in0 : (a == 1 ? in1 : in2));
+      xfft_line<N, false>(s_w, s_tw, tid);
+#pragma unroll
+      for (int i = 0; i < XEPT; ++i) {  // conj(S_a) = +i D_a green:  q += i m_a (re + i im)
+        const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
+        const float dm = a == 0 ? (float)t.grad[kx] : (a == 1 ? dyv : dzv);
+        const float2 d = s_w[sidx(p, c)];
+        float2 acc = a == 0 ? make_float2(0.f, 0.f) : s_a[sidx(p, c)];
+        acc.x -= dm * d.y;
+        acc.y += dm * d.x;
+        s_a[sidx(p, c)] = acc;
+      }
+      __syncthreads();
+    }
+#pragma unroll 1
+    for (int o = 0; o < (two ? 2 : 1); ++o) {
+#pragma unroll
+      for (int i = 0; i < XEPT; ++i) {
+        const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
+        const float g = (float)green_of(kx) * (two ? 0.5f : 1.0f);
+        const float2 d = s_a[sidx(p, c)];
+        float2 v = make_float2(g * d.x, g * d.y);
+        if (o == 1) {  // conj of the interlace phase
+          const float2 ph = phase_of(kx);
+          v = cmulc(v, ph);
+        }
+        s_w[sidx(p, c)] = v;
+      }
+      __syncthreads();
+      xfft_line<N, true>(s_w, s_tw, tid);
+      store_line(o == 0 ? out0 : out1);
+    }
+  }
+}
+
+// ---- host side -------------------------------------------------------------------------------------------
+bool xfft_supported(int m) { return m == 64 || m == 128 || m == 256 || m == 512 || m == 1024; }
+
+int xfft_init(Ctx* c) {  // twiddle table and the batched 2-D (y,z) cuFFT plans; called from pm_create
+  c->xfused = false;
+  if (!xfft_supported(c->mg)) return PM_OK;
+  const char* off = getenv("PMF_NO_XFUSE");  // A/B switch for measurements and for testing the unfused path
+  if (off && atoi(off)) return PM_OK;
+  const int m = c->mg;
+  std::vector<float2> tw(m);
+  for (int k = 0; k < m; ++k) {
+    const double a = -2.0 * M_PI * (double)k / (double)m;
+    tw[k] = make_float2((float)cos(a), (float)sin(a));
+  }
+  PM_CUDA(c, cudaMalloc((void**)&c->xtw, sizeof(float2) * (size_t)m));
+  PM_CUDA(c, cudaMemcpy(c->xtw, tw.data(), sizeof(float2) * (size_t)m, cudaMemcpyHostToDevice));
+  int n2[2] = {m, m};
+  size_t ws1 = 0, ws2 = 0;
+  PM_CUFFT(c, cufftCreate(&c->plan2_r2c));
+  PM_CUFFT(c, cufftCreate(&c->plan2_c2r));
+  c->plans2_ok = true;
+  PM_CUFFT(c, cufftSetAutoAllocation(c->plan2_r2c, 0));
+  PM_CUFFT(c, cufftSetAutoAllocation(c->plan2_c2r, 0));
+  PM_CUFFT(c, cufftMakePlanMany(c->plan2_r2c, 2, n2, nullptr, 1, 0, nullptr, 1, 0, CUFFT_R2C, m, &ws1));
+  PM_CUFFT(c, cufftMakePlanMany(c->plan2_c2r, 2, n2, nullptr, 1, 0, nullptr, 1, 0, CUFFT_C2R, m, &ws2));
+  c->fft2_work_bytes = ws1 > ws2 ? ws1 : ws2;
+  c->xfused = true;
+  return PM_OK;
+}
+
+int fft2_r2c(Ctx* c, const float* in, float2* out, cudaStream_t st) {
+  PM_CUFFT(c, cufftSetStream(c->plan2_r2c, st));
+  PM_CUFFT(c, cufftExecR2C(c->plan2_r2c, const_cast<float*>(in), reinterpret_cast<cufftComplex*>(out)));
+  return PM_OK;
+}
+int fft2_c2r(Ctx* c, float2* in, float* out, cudaStream_t st) {
+  PM_CUFFT(c, cufftSetStream(c->plan2_c2r, st));
+  PM_CUFFT(c, cufftExecC2R(c->plan2_c2r, reinterpret_cast<cufftComplex*>(in), out));
+  return PM_OK;
+}
+
+template <int N, int MODE>
+static int xfft_launch_n(Ctx* c, const XTabs& t, const float2* i0, const float2* i1, const float2* i2, float2* o0,
+                         float2* o1, float2* o2, double coeff_eff, cudaStream_t st) {
+  constexpr int NT = N * XC / XEPT;
+  constexpr size_t smem = sizeof(float2) * 2 * (size_t)xfft_smem_elems<N>();
+  auto kern = k_xfft_kspace<N, MODE>;
+  static bool attr = false;
+  if (!attr) {
+    PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr = true;
+  }
+  const int64_t grid = (t.ncol + XC - 1) / XC;
+  kern<<<(unsigned)grid, NT, smem, st>>>(t, i0, i1, i2, o0, o1, o2, coeff_eff);
+  count_launch(c);
+  PM_CUDA(c, cudaGetLastError());
+  return PM_OK;
+}
+
+template <int MODE>
+static int xfft_launch(Ctx* c, const float2* i0, const float2* i1, const float2* i2, float2* o0, float2* o1,
+                       float2* o2, double coeff_eff, cudaStream_t st) {
+  XTabs t;
+  t.grad = c->tab_grad;
+  t.lap = c->tab_lap;
+  t.win = c->tab_win;
+  t.pc = c->tab_cos;
+  t.ps = c->tab_sin;
+  t.tw = c->xtw;
+  t.m = c->mg;
+  t.hz = c->mg / 2 + 1;
+  t.ncol = (int64_t)t.m * t.hz;
+  switch (c->mg) {
+    case 64: return xfft_launch_n<64, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
+    case 128: return xfft_launch_n<128, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
+    case 256: return xfft_launch_n<256, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
+    case 512: return xfft_launch_n<512, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
+    case 1024: return xfft_launch_n<1024, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
+  }
+  return fail(c, PM_ESTATE, "fused x-FFT not built for m = %d", c->mg);
+}
+
+// d1 (, d2): (y,z)-transformed density spectra -> gh[a]: x-inverse-transformed force spectra
+int launch_xfft_forward(Ctx* c, const float2* d1, const float2* d2, float2* const gh[3], double coeff_eff,
+                        cudaStream_t st) {
+  return xfft_launch<0>(c, d1, d2, nullptr, gh[0], gh[1], gh[2], coeff_eff, st);
+}
+// gh[a]: (y,z)-transformed cotangent spectra -> q1 (, q2): x-inverse-transformed density cotangent spectra
+int launch_xfft_transpose(Ctx* c, const float2* const gh[3], float2* q1, float2* q2, double coeff_eff,
+                          cudaStream_t st) {
+  return xfft_launch<1>(c, gh[0], gh[1], gh[2], q1, q2, nullptr, coeff_eff, st);
+}
+
+// ---- the spectral operator on real meshes, fused or not ------------------------------------------------------
+int spectral_forward(Ctx* c, const float* d1, const float* d2, float* const g[3], double coeff_eff, bool stages,
+                     cudaStream_t st) {
+  const bool fused = c->xfused;
+  if (stages) stage_begin(c, PM_STAGE_FFT_FWD, st);
+  PM_TRY(fused ? fft2_r2c(c, d1, c->dhat[0], st) : fft_r2c(c, d1, c->dhat[0], st));
+  if (d2) PM_TRY(fused ? fft2_r2c(c, d2, c->dhat[1], st) : fft_r2c(c, d2, c->dhat[1], st));
+  if (stages) stage_end(c, PM_STAGE_FFT_FWD, st);
+  if (stages) stage_begin(c, PM_STAGE_KSPACE, st);
+  if (fused)
+    PM_TRY(launch_xfft_forward(c, c->dhat[0], d2 ? c->dhat[1] : nullptr, c->ghat, coeff_eff, st));
+  else
+    PM_TRY(launch_kspace_forward(c, c->dhat[0], d2 ? c->dhat[1] : nullptr, c->ghat, coeff_eff, st));
+  if (stages) stage_end(c, PM_STAGE_KSPACE, st);
+  if (stages) stage_begin(c, PM_STAGE_FFT_INV, st);
+  for (int a = 0; a < 3; ++a) PM_TRY(fused ? fft2_c2r(c, c->ghat[a], g[a], st) : fft_c2r(c, c->ghat[a], g[a], st));
+  if (stages) stage_end(c, PM_STAGE_FFT_INV, st);
+  return PM_OK;
+}
+
+int spectral_transpose(Ctx* c, const float* const gb[3], float* q1, float* q2, double coeff_eff, cudaStream_t st) {
+  const bool fused = c->xfused;
+  for (int a = 0; a < 3; ++a) PM_TRY(fused ? fft2_r2c(c, gb[a], c->ghat[a], st) : fft_r2c(c, gb[a], c->ghat[a], st));
+  if (fused)
+    PM_TRY(launch_xfft_transpose(c, c->ghat, c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, st));
+  else
+    PM_TRY(launch_kspace_transpose(c, c->ghat, c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, st));
+  PM_TRY(fused ? fft2_c2r(c, c->dhat[0], q1, st) : fft_c2r(c, c->dhat[0], q1, st));
+  if (q2) PM_TRY(fused ? fft2_c2r(c, c->dhat[1], q2, st) : fft_c2r(c, c->dhat[1], q2, st));
+  return PM_OK;
+}
+
+}  // namespace pmf

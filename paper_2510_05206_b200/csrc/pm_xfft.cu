@@ -112,7 +112,7 @@ struct Dft<16, SIGN> {
 // ---- shared-memory line layout and the FFT stages -----------------------------------------------------------
 // Element (x position p, column c) sits at float2 index p * XC + c + 8 * (p / 8): a row of 8 columns is half of
 // the 32 banks; the padding puts rows p and p + 8 (last stage) in different halves, rows p and p + 1 are anyway.
-__device__ __forceinline__ int sidx(int p, int c) { return p * XC + c + ((p >> 3) << 3); }
+__device__ __forceinline__ int sidx(int p, int c) { return 9 * p - (p & 7) + c; }  // = 8 p + c + 8 (p / 8), XC = 8
 template <int N>
 constexpr int xfft_smem_elems() { return N * XC + (N / 8) * 8; }
 
@@ -126,8 +126,12 @@ template <> struct Radices<1024> { static constexpr int r0 = 16, r1 = 8,  r2 = 8
 
 // One radix-R stage over sub-transforms of size S (M = S / R butterflies each).  tw[k] = e^{-2 pi i k / N}.
 //   forward (DIF): y = DFT_R(x), y_q *= W_S^{jq};      inverse (DIT): x_r *= conj(W_S)^{jr}, y = IDFT_R(x)
-template <int N, int R, int S, bool INV>
-__device__ __forceinline__ void xfft_stage(float2* s, const float2* tw, int tid) {
+// ld(p, c) / st(p, c, v) read and write element (position p, column c): the shared-memory line for the inner
+// stages; the first load and the last store of a transform go straight from / to global memory or carry the
+// pointwise k-space factors, which saves four of the nine passes over shared memory per transform (the kernel is
+// bound by shared-memory bandwidth).  A thread's column c is the same in every stage.
+template <int N, int R, int S, bool INV, class Ld, class St>
+__device__ __forceinline__ void xfft_stage(const float2* __restrict__ tw, int tid, Ld ld, St st) {
   constexpr int M = S / R, NB = N * XC / R, NT = N * XC / XEPT;
 #pragma unroll
   for (int b = tid; b < NB; b += NT) {
@@ -135,34 +139,50 @@ __device__ __forceinline__ void xfft_stage(float2* s, const float2* tw, int tid)
     const int p0 = blk * S + j;
     float2 v[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) v[r] = s[sidx(p0 + r * M, c)];
+    for (int r = 0; r < R; ++r) v[r] = ld(p0 + r * M, c);
     if (INV) {
+      if (M > 1)  // M = 1: j = 0, every twiddle is 1
 #pragma unroll
-      for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], __ldg(tw + (N / S) * j * r));
+        for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], __ldg(tw + (N / S) * j * r));
       Dft<R, 1>::run(v);
     } else {
       Dft<R, -1>::run(v);
+      if (M > 1)
 #pragma unroll
-      for (int q = 1; q < R; ++q) v[q] = cmulx(v[q], __ldg(tw + (N / S) * j * q));
+        for (int q = 1; q < R; ++q) v[q] = cmulx(v[q], __ldg(tw + (N / S) * j * q));
     }
 #pragma unroll
-    for (int q = 0; q < R; ++q) s[sidx(p0 + q * M, c)] = v[q];
+    for (int q = 0; q < R; ++q) st(p0 + q * M, c, v[q]);
   }
   __syncthreads();
 }
 
-template <int N, bool INV>
-__device__ __forceinline__ void xfft_line(float2* s, const float2* tw, int tid) {
+// A whole transform of the line in s: `first` loads the input of the first stage, `last` stores the output of
+// the last stage (forward: element at position p holds frequency xfft_freq(p); inverse: natural order).
+template <int N, bool INV, class Ld, class St>
+__device__ __forceinline__ void xfft_line(float2* s, const float2* __restrict__ tw, int tid, Ld first, St last) {
   using Rd = Radices<N>;
   constexpr int S1 = N / Rd::r0, S2 = S1 / Rd::r1;
+  constexpr bool three = Rd::r2 > 1;
+  constexpr int R2 = three ? Rd::r2 : 8, S2e = three ? S2 : 8;  // (a valid, unused instantiation when r2 = 1)
+  auto lds = [s](int p, int c) { return s[sidx(p, c)]; };
+  auto sts = [s](int p, int c, float2 v) { s[sidx(p, c)] = v; };
   if (!INV) {
-    xfft_stage<N, Rd::r0, N, false>(s, tw, tid);
-    xfft_stage<N, Rd::r1, S1, false>(s, tw, tid);
-    if (Rd::r2 > 1) xfft_stage<N, (Rd::r2 > 1 ? Rd::r2 : 8), (Rd::r2 > 1 ? S2 : 8), false>(s, tw, tid);
+    xfft_stage<N, Rd::r0, N, false>(tw, tid, first, sts);
+    if (three) {
+      xfft_stage<N, Rd::r1, S1, false>(tw, tid, lds, sts);
+      xfft_stage<N, R2, S2e, false>(tw, tid, lds, last);
+    } else {
+      xfft_stage<N, Rd::r1, S1, false>(tw, tid, lds, last);
+    }
   } else {
-    if (Rd::r2 > 1) xfft_stage<N, (Rd::r2 > 1 ? Rd::r2 : 8), (Rd::r2 > 1 ? S2 : 8), true>(s, tw, tid);
-    xfft_stage<N, Rd::r1, S1, true>(s, tw, tid);
-    xfft_stage<N, Rd::r0, N, true>(s, tw, tid);
+    if (three) {
+      xfft_stage<N, R2, S2e, true>(tw, tid, first, sts);
+      xfft_stage<N, Rd::r1, S1, true>(tw, tid, lds, sts);
+    } else {
+      xfft_stage<N, Rd::r1, S1, true>(tw, tid, first, sts);
+    }
+    xfft_stage<N, Rd::r0, N, true>(tw, tid, lds, last);
   }
 }
 
@@ -188,17 +208,15 @@ struct XTabs {
 //   MODE 1 (transpose): in0..2 -> out0 (, out1) = x-inverse of sum_a conj(S_a) ghat_a
 // Every input is the (y,z)-transformed, x-untransformed spectrum [x][y][hz]; every output likewise.
 template <int N, int MODE>
-__global__ void __launch_bounds__(N* XC / XEPT) k_xfft_kspace(XTabs t, const float2* __restrict__ in0,
+__global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? 3 : 1) k_xfft_kspace(XTabs t, const float2* __restrict__ in0,
                                                                const float2* __restrict__ in1,
                                                                const float2* __restrict__ in2,
                                                                float2* __restrict__ out0, float2* __restrict__ out1,
                                                                float2* __restrict__ out2, double coeff_eff) {
-  constexpr int NT = N * XC / XEPT;
   constexpr int SE = xfft_smem_elems<N>();
   extern __shared__ __align__(16) float2 s_x[];
   float2* s_w = s_x;        // work line: FFT in place
   float2* s_a = s_x + SE;   // MODE 0: green * dhat;  MODE 1: accumulated q
-  const float2* s_tw = t.tw;  // 8 m bytes, read through L1 (keeps three 512-point CTAs per SM)
   const int tid = threadIdx.x;
   const int c = tid % XC;   // this thread's column in every pointwise loop (NT is a multiple of XC)
   const int64_t q = (int64_t)blockIdx.x * XC + c;
@@ -206,24 +224,14 @@ __global__ void __launch_bounds__(N* XC / XEPT) k_xfft_kspace(XTabs t, const flo
   const int iy = live ? (int)(q / t.hz) : 0, iz = live ? (int)(q - (int64_t)iy * t.hz) : 0;
   const size_t plane = (size_t)t.ncol;
 
-  auto load_line = [&](const float2* __restrict__ src) {
-    float2 v[XEPT];
-#pragma unroll
-    for (int i = 0; i < XEPT; ++i) {
-      const int p = tid / XC + i * (NT / XC);
-      v[i] = live ? __ldcs(src + (size_t)p * plane + q) : make_float2(0.f, 0.f);
-    }
-#pragma unroll
-    for (int i = 0; i < XEPT; ++i) s_w[sidx(tid / XC + i * (NT / XC), c)] = v[i];
-    __syncthreads();
+  // global memory as the first load / last store of a transform (64 contiguous bytes per x plane and CTA)
+  auto gld = [&](const float2* __restrict__ src) {
+    return [=](int p, int) { return live ? __ldcs(src + (size_t)p * plane + q) : make_float2(0.f, 0.f); };
   };
-  auto store_line = [&](float2* __restrict__ dst) {  // after the inverse stages (they end with a barrier)
-#pragma unroll
-    for (int i = 0; i < XEPT; ++i) {
-      const int p = tid / XC + i * (NT / XC);
-      if (live) dst[(size_t)p * plane + q] = s_w[sidx(p, c)];
-    }
-    __syncthreads();
+  auto gst = [&](float2* __restrict__ dst) {
+    return [=](int p, int, float2 v) {
+      if (live) dst[(size_t)p * plane + q] = v;
+    };
   };
 
   // column factors
@@ -231,89 +239,71 @@ __global__ void __launch_bounds__(N* XC / XEPT) k_xfft_kspace(XTabs t, const flo
   const float dyv = (float)t.grad[iy], dzv = (float)t.grad[iz];
   const double pcyz = t.pc[iy] * t.pc[iz] - t.ps[iy] * t.ps[iz], psyz = t.pc[iy] * t.ps[iz] + t.ps[iy] * t.pc[iz];
 
-  auto green_of = [&](int kx) -> double {  // coeff / (Lap * window); 0 at n = 0 and for dropped modes
+  auto green_of = [&](int kx) -> float {  // coeff / (Lap * window); 0 at n = 0 and for dropped modes
     const double den = (lyz + t.lap[kx]) * (wyz * t.win[kx]);
-    return den != 0.0 ? coeff_eff / den : 0.0;
+    return den != 0.0 ? (float)(coeff_eff / den) : 0.0f;
   };
   auto phase_of = [&](int kx) -> float2 {  // interlace phase e^{-ik.s} (real part only on Nyquist planes, R9)
     return make_float2((float)(t.pc[kx] * pcyz - t.ps[kx] * psyz), (float)(t.pc[kx] * psyz + t.ps[kx] * pcyz));
   };
+  auto grad_of = [&](int a, int kx) -> float { return a == 0 ? (float)t.grad[kx] : (a == 1 ? dyv : dzv); };
 
+  // In every transform the last forward stage and the first inverse stage give a thread the same elements
+  // (same radix, same sub-transform size), so s_a is only ever touched by the thread that owns the element.
   if (MODE == 0) {
     const bool two = in1 != nullptr;
-    if (two) {  // second grid first: s_a = 1/2 phase * dhat2
-      load_line(in1);
-      xfft_line<N, false>(s_w, s_tw, tid);
-#pragma unroll
-      for (int i = 0; i < XEPT; ++i) {
-        const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
-        const float2 e = cmulx(phase_of(kx), s_w[sidx(p, c)]);
-        s_a[sidx(p, c)] = make_float2(0.5f * e.x, 0.5f * e.y);
-      }
-      __syncthreads();
-    }
-    load_line(in0);
-    xfft_line<N, false>(s_w, s_tw, tid);
-#pragma unroll
-    for (int i = 0; i < XEPT; ++i) {  // s_a = green * dhat (each thread touches only its own elements of s_a)
-      const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
-      float2 d = s_w[sidx(p, c)];
+    if (two)  // second grid first: s_a = 1/2 phase * dhat2
+      xfft_line<N, false>(s_w, t.tw, tid, gld(in1), [&](int p, int cc, float2 v) {
+        const float2 e = cmulx(phase_of(xfft_freq<N>(p)), v);
+        s_a[sidx(p, cc)] = make_float2(0.5f * e.x, 0.5f * e.y);
+      });
+    xfft_line<N, false>(s_w, t.tw, tid, gld(in0), [&](int p, int cc, float2 v) {  // s_a = green * dhat
       if (two) {
-        const float2 e = s_a[sidx(p, c)];
-        d = make_float2(0.5f * d.x + e.x, 0.5f * d.y + e.y);
+        const float2 e = s_a[sidx(p, cc)];
+        v = make_float2(0.5f * v.x + e.x, 0.5f * v.y + e.y);
       }
-      const float g = (float)green_of(kx);
-      s_a[sidx(p, c)] = make_float2(g * d.x, g * d.y);
-    }
-    __syncthreads();
+      const float g = green_of(xfft_freq<N>(p));
+      s_a[sidx(p, cc)] = make_float2(g * v.x, g * v.y);
+    });
 #pragma unroll 1
     for (int a = 0; a < 3; ++a) {
-#pragma unroll
-      for (int i = 0; i < XEPT; ++i) {  // -i D_a (re + i im) = D_a (im - i re)
-        const int p = tid / XC + i * (NT / XC);
-        const float dm = a == 0 ? (float)t.grad[xfft_freq<N>(p)] : (a == 1 ? dyv : dzv);
-        const float2 d = s_a[sidx(p, c)];
-        s_w[sidx(p, c)] = make_float2(dm * d.y, -dm * d.x);
-      }
-      __syncthreads();
-      xfft_line<N, true>(s_w, s_tw, tid);
-      store_line(a == 0 ? out0 : (a == 1 ? out1 : out2));
+      float2* dst = a == 0 ? out0 : (a == 1 ? out1 : out2);
+      xfft_line<N, true>(
+          s_w, t.tw, tid,
+          [&](int p, int cc) {  // -i D_a (re + i im) = D_a (im - i re)
+            const float dm = grad_of(a, xfft_freq<N>(p));
+            const float2 d = s_a[sidx(p, cc)];
+            return make_float2(dm * d.y, -dm * d.x);
+          },
+          gst(dst));
     }
   } else {
     const bool two = out1 != nullptr;
 #pragma unroll 1
     for (int a = 0; a < 3; ++a) {
-      load_line(a == 0 ? in0 : (a == 1 ? in1 : in2));
-      xfft_line<N, false>(s_w, s_tw, tid);
-#pragma unroll
-      for (int i = 0; i < XEPT; ++i) {  // conj(S_a) = +i D_a green:  q += i m_a (re + i im)
-        const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
-        const float dm = a == 0 ? (float)t.grad[kx] : (a == 1 ? dyv : dzv);
-        const float2 d = s_w[sidx(p, c)];
-        float2 acc = a == 0 ? make_float2(0.f, 0.f) : s_a[sidx(p, c)];
-        acc.x -= dm * d.y;
-        acc.y += dm * d.x;
-        s_a[sidx(p, c)] = acc;
-      }
-      __syncthreads();
+      const float2* src = a == 0 ? in0 : (a == 1 ? in1 : in2);
+      xfft_line<N, false>(s_w, t.tw, tid, gld(src), [&](int p, int cc, float2 v) {
+        // conj(S_a) = +i D_a green:  q += i D_a (re + i im); green is applied on the way out
+        const float dm = grad_of(a, xfft_freq<N>(p));
+        float2 acc = a == 0 ? make_float2(0.f, 0.f) : s_a[sidx(p, cc)];
+        acc.x -= dm * v.y;
+        acc.y += dm * v.x;
+        s_a[sidx(p, cc)] = acc;
+      });
     }
 #pragma unroll 1
     for (int o = 0; o < (two ? 2 : 1); ++o) {
-#pragma unroll
-      for (int i = 0; i < XEPT; ++i) {
-        const int p = tid / XC + i * (NT / XC), kx = xfft_freq<N>(p);
-        const float g = (float)green_of(kx) * (two ? 0.5f : 1.0f);
-        const float2 d = s_a[sidx(p, c)];
-        float2 v = make_float2(g * d.x, g * d.y);
-        if (o == 1) {  // conj of the interlace phase
-          const float2 ph = phase_of(kx);
-          v = cmulc(v, ph);
-        }
-        s_w[sidx(p, c)] = v;
-      }
-      __syncthreads();
-      xfft_line<N, true>(s_w, s_tw, tid);
-      store_line(o == 0 ? out0 : out1);
+      xfft_line<N, true>(
+          s_w, t.tw, tid,
+          [&](int p, int cc) {
+            const int kx = xfft_freq<N>(p);
+            const float g = green_of(kx) * (two ? 0.5f : 1.0f);
+            const float2 d = s_a[sidx(p, cc)];
+            float2 v = make_float2(g * d.x, g * d.y);
+            if (o == 1) v = cmulc(v, phase_of(kx));  // conj of the interlace phase
+            return v;
+          },
+          gst(o == 0 ? out0 : out1));
     }
   }
 }

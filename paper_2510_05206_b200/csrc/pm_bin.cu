@@ -15,6 +15,7 @@ namespace pmf {
 
 struct BinGeom {
   int m, ntx, nty, ntz, xbl;
+  int fast_tiles;    // m is a multiple of every tile edge: the box edge is a tile boundary (see tile_fast)
   float c_hi, c_lo;  // m / box split into two floats (c_hi + c_lo = m/box to ~2^-48)
   double inv_dx;     // m / box
 };
@@ -59,13 +60,32 @@ __device__ __forceinline__ uint32_t tile_and_local(float x, float y, float z, co
   return tile_id(tx, ty, tz, g.nty, g.ntz, g.xbl);
 }
 
-__device__ __forceinline__ uint32_t tile_only(float x, float y, float z, const BinGeom& g) {
+__device__ __forceinline__ uint32_t tile_exact(float x, float y, float z, const BinGeom& g) {
   int cx, cy, cz;
   uint32_t f;
   cell_coord(x, g, cx, f);
   cell_coord(y, g, cy, f);
   cell_coord(z, g, cz, f);
   return tile_id(cx / TX, cy / TY, cz / TZ, g.nty, g.ntz, g.xbl);
+}
+
+// Histogram pass: only the tile is needed.  v = x * (m/L)/T is u/T to ~1e-5 tiles in plain fp32; unless v lies
+// within 1e-3 of a tile boundary (or outside the box) floor(v) IS the tile the exact coordinate gives, and
+// the pass skips the error-free product (it is issue-bound: ncu 70 % issue active, 40 % of HBM).  The rare
+// boundary cases take the exact path, so both passes always agree.
+__device__ __forceinline__ bool tile_fast(float x, float ct, int nt, int& t) {
+  const float vm = __fmaf_rn(x, ct, -0.5f);
+  const float tt = __fadd_rn(vm, 12582912.0f);  // 1.5 * 2^23: nearest integer to v - 1/2 in the low mantissa bits
+  t = __float_as_int(tt) - 0x4B400000;
+  const float r = __fsub_rn(vm, __fsub_rn(tt, 12582912.0f));  // v - (t + 1/2), in [-1/2, 1/2]
+  return fabsf(r) < 0.499f && (unsigned)t < (unsigned)nt;
+}
+__device__ __forceinline__ uint32_t tile_only(float x, float y, float z, const BinGeom& g) {
+  int tx, ty, tz;
+  const bool ok = tile_fast(x, g.c_hi * (1.0f / TX), g.ntx, tx) & tile_fast(y, g.c_hi * (1.0f / TY), g.nty, ty) &
+                  tile_fast(z, g.c_hi * (1.0f / TZ), g.ntz, tz);
+  if (!ok || !g.fast_tiles) return tile_exact(x, y, z, g);
+  return tile_id(tx, ty, tz, g.nty, g.ntz, g.xbl);
 }
 
 // The lanes of a warp hold 32 CONSECUTIVE particles.  Each run of equal keys elects its first lane, which
@@ -332,6 +352,7 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   g.nty = c->nty;
   g.ntz = c->ntz;
   g.xbl = c->xbl;
+  g.fast_tiles = (c->mg % TX == 0 && c->mg % TY == 0 && c->mg % TZ == 0) ? 1 : 0;
   g.inv_dx = (double)c->mg / c->p.box;
   g.c_hi = (float)g.inv_dx;
   g.c_lo = (float)(g.inv_dx - (double)g.c_hi);
@@ -343,10 +364,11 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   // persistent grid: resident CTAs per SM (register-limited) x SMs, capped by the work
   const int64_t work = aligned ? (N + BIN_WARP_PART - 1) / BIN_WARP_PART : (N + 31) / 32;  // warp iterations
   int grid = (int)((work + BIN_BLOCK / 32 - 1) / (BIN_BLOCK / 32));
-  const int gmax = c->num_sms * c->bin_occ;
-  if (grid > gmax) grid = gmax;
   if (grid < 1) grid = 1;
-  if (N > 0) k_bin_pass<false><<<grid, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, nullptr, aligned);
+  int grid0 = grid;  // the histogram pass needs fewer registers: its own residency
+  if (grid > c->num_sms * c->bin_occ) grid = c->num_sms * c->bin_occ;
+  if (grid0 > c->num_sms * c->bin_occ0) grid0 = c->num_sms * c->bin_occ0;
+  if (N > 0) k_bin_pass<false><<<grid0, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, nullptr, aligned);
   k_scan_reduce<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial);
   k_scan_partials<<<1, SCAN_T, 0, st>>>(partial, nb, c->tile_off, c->item_off, nt, c->nitems);
   k_scan_final<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, c->tile_off, c->item_off);
@@ -361,11 +383,12 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   return PM_OK;
 }
 
-int bin_occupancy() {
-  int a = 0, b = 0;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_bin_pass<false>, BIN_BLOCK, 0);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_bin_pass<true>, BIN_BLOCK, 0);
-  const int o = a < b ? a : b;
+int bin_occupancy(int pass) {
+  int o = 0;
+  if (pass == 0)
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_bin_pass<false>, BIN_BLOCK, 0);
+  else
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_bin_pass<true>, BIN_BLOCK, 0);
   return o < 1 ? 1 : o;
 }
 

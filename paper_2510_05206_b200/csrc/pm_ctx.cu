@@ -226,7 +226,8 @@ static int build(Ctx* c) {
   c->nty = (mg + TY - 1) / TY;
   c->ntz = (mg + TZ - 1) / TZ;
   c->ntiles = c->ntx * c->nty * c->ntz;
-  c->bin_occ = bin_occupancy();
+  c->bin_occ0 = bin_occupancy(0);
+  c->bin_occ = bin_occupancy(1);
   c->xbl = (c->ntx % 8 == 0) ? 3 : (c->ntx % 4 == 0) ? 2 : (c->ntx % 2 == 0) ? 1 : 0;
 
   // tables
@@ -308,7 +309,7 @@ static void teardown(Ctx* c) {
   void* ptrs[] = {c->tab_grad, c->tab_lap, c->tab_win, c->tab_cos, c->tab_sin, c->rec, c->tile_cnt,
                   c->tile_off, c->item_off, c->scan_tmp, c->items, c->nitems, c->sched, c->fft_work, c->rho[0],
                   c->rho[1], c->dhat[0], c->dhat[1], c->ghat[0], c->ghat[1], c->ghat[2], c->g[0],
-                  c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->xtw, c->host_pos_dev,
+                  c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->xtw, c->xsym, c->xph, c->host_pos_dev,
                   c->host_force_dev};
   for (void* q : ptrs)
     if (q) cudaFree(q);

@@ -222,13 +222,25 @@ __device__ __forceinline__ void sched_done(uint32_t* sched) {
 }
 
 // record loads: read once per kernel -> streaming (evict-first) so they do not push mesh tiles out of L2
-__device__ __forceinline__ uint4 load_rec(const uint4* p) { return __ldcs(p); }
+template <bool IDX>  // IDX: the caller reads the original index (.w)
+__device__ __forceinline__ void load_rec(uint4& r, const BinView& bv, uint32_t i) {
+  r = __ldcs(bv.rec + i);
+}
 
 // ---- K2 / K5: tile scatter ---------------------------------------------------------------------------
-// Persistent CTAs draw work items from the dynamic schedule.  The accumulator tile is zeroed once; every
-// flush writes zeros back, so a work item costs two barriers.  roll is in [0, m).
+// Persistent CTAs draw work items from the dynamic schedule, two items ahead: while item i is deposited, the
+// records of item i+1 are already being loaded into the registers item i frees (rolling prefetch), and its
+// WorkItem was fetched during the flush of item i-1.  The accumulator tile is zeroed once; every flush writes
+// zeros back.  With NBUF = 2 accumulator tiles the flush of item i and the deposit of item i+1 use different
+// buffers, so a work item costs ONE barrier (ncu before: barrier 33 %, long scoreboard 28 % of the stall
+// cycles with two barriers and loads issued after the deposit).  roll is in [0, m).
+// resident CTAs per SM the register allocation aims at (the unit-weight CIC assign is the headline kernel)
 template <class T, int NCOMP, bool WEIGHTED>
-__global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Params tp, int3 roll,
+constexpr int scatter_min_ctas() {
+  return (NCOMP == 1 && !WEIGHTED) ? (T::P == 2 ? 4 : (T::P <= 4 ? 3 : 1)) : (NCOMP == 1 ? 2 : 1);
+}
+template <class T, int NCOMP, bool WEIGHTED, int NBUF>
+__global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>()) k_scatter(BinView bv, typename T::Params tp, int3 roll,
                                                    const float* __restrict__ wsrc, int wstride,
                                                    MeshPtrs<NCOMP> mesh) {
   using G = Geo<T>;
@@ -236,14 +248,16 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
   constexpr int NG = NCOMP * G::NGROUP;                          // groups to flush
   constexpr int NSLOT = (NG + BLOCK - 1) / BLOCK;                // groups per thread
   constexpr bool PRE = NSLOT <= 6;                               // group coordinates kept in registers
-  extern __shared__ __align__(16) int s_acc[];
+  constexpr int ACC = NCOMP * G::COMP;                           // words per accumulator buffer
+  extern __shared__ __align__(16) int s_acc_all[];
   __shared__ float s_red[(BLOCK / 32) * NCOMP];
   __shared__ uint32_t s_next[2];
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
 
-  for (int j = tid; j < NCOMP * G::COMP / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
+  for (int j = tid; j < NBUF * ACC / 4; j += BLOCK) reinterpret_cast<int4*>(s_acc_all)[j] = make_int4(0, 0, 0, 0);
+  if (tid == 0) s_next[0] = sched_next(bv.sched);  // the item after this CTA's first
 
   // (comp, sx, sy, z offset) of the groups this thread flushes, packed 4 | 8 | 8 | 12 bits
   auto group_coords = [](int j) -> uint32_t {
@@ -260,29 +274,31 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
   }
   __syncthreads();
 
-  // records of a work item -> registers.  The next item's records are requested right after the deposit
-  // loop, so their latency is covered by the flush of the current tile.
-  WorkItem wi;
+  // records of a work item -> registers
+  WorkItem wi, nwi;
+  wi.begin = wi.end = wi.txyz = nwi.begin = nwi.end = nwi.txyz = 0;
   uint4 r[PPT];
   auto load_batch = [&](uint32_t b0, uint32_t end) {  // up to CHUNK records starting at b0
 #pragma unroll
     for (int k = 0; k < PPT; ++k) {
       const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
-      if (i < end) r[k] = load_rec(bv.rec + i);
+      if (i < end) load_rec<WEIGHTED>(r[k], bv, i);
     }
   };
-  auto load_item = [&](uint32_t id) {
-    wi = bv.items[id];
+  uint32_t it = blockIdx.x, nxt = s_next[0];
+  int par = 1;
+  int* s_acc = s_acc_all;
+  if (it < nitems) {
+    wi = bv.items[it];
     load_batch(wi.begin, wi.end);
-  };
-  uint32_t it = blockIdx.x;
-  int par = 0;
-  if (it < nitems) load_item(it);
+  }
+  if (nxt < nitems) nwi = bv.items[nxt];
   while (it < nitems) {
-    if (tid == 0) s_next[par] = sched_next(bv.sched);
+    if (tid == 0) s_next[par] = sched_next(bv.sched);  // item i+2
     const uint32_t n = wi.end - wi.begin;
     const uint32_t ibegin = wi.begin, iend = wi.end;
     const TileOrigin o = tile_origin(wi);
+    const uint32_t nbegin = nwi.begin, nend = nxt < nitems ? nwi.end : nwi.begin;  // empty when there is no next item
 
     float wv[PPT][NCOMP];
     float wabs[NCOMP];
@@ -350,51 +366,57 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
     }
 
     for (uint32_t b0 = ibegin;;) {
+      const bool last = b0 + CHUNK >= iend;  // uniform
 #pragma unroll
-    for (int k = 0; k < PPT; ++k) {
-      const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
-      if (i < iend) {
-        int sx, sy, sz;
-        float wx[P], wy[P], wz[P], dummy[P];
-        T::template axis<false>(apply_shift<T>(r[k].x, tp.frac[0]), tp, sx, wx, dummy);
-        T::template axis<false>(apply_shift<T>(r[k].y, tp.frac[1]), tp, sy, wy, dummy);
-        T::template axis<false>(apply_shift<T>(r[k].z, tp.frac[2]), tp, sz, wz, dummy);
-        NodeCol nc[P];
+      for (int k = 0; k < PPT; ++k) {
+        const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
+        if (i < iend) {
+          int sx, sy, sz;
+          float wx[P], wy[P], wz[P], dummy[P];
+          T::template axis<false>(apply_shift<T>(r[k].x, tp.frac[0]), tp, sx, wx, dummy);
+          T::template axis<false>(apply_shift<T>(r[k].y, tp.frac[1]), tp, sy, wy, dummy);
+          T::template axis<false>(apply_shift<T>(r[k].z, tp.frac[2]), tp, sz, wz, dummy);
+          NodeCol nc[P];
 #pragma unroll
-        for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
-        float wzs[NCOMP][P];  // the scale (and the particle's weight) folded into the z weights
+          for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
+          float wzs[NCOMP][P];  // the scale (and the particle's weight) folded into the z weights
 #pragma unroll
-        for (int q = 0; q < NCOMP; ++q)
+          for (int q = 0; q < NCOMP; ++q)
 #pragma unroll
-          for (int c = 0; c < P; ++c) wzs[q][c] = wz[c] * (wv[k][q] * scale[q]);
+            for (int c = 0; c < P; ++c) wzs[q][c] = wz[c] * (wv[k][q] * scale[q]);
 #pragma unroll
-        for (int a = 0; a < P; ++a)
+          for (int a = 0; a < P; ++a)
 #pragma unroll
-          for (int b = 0; b < P; ++b) {
-            const float wxy = wx[a] * wy[b];
+            for (int b = 0; b < P; ++b) {
+              const float wxy = wx[a] * wy[b];
 #pragma unroll
-            for (int c = 0; c < P; ++c) {
-              int* node = s_acc + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
+              for (int c = 0; c < P; ++c) {
+                int* node = s_acc + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
 #pragma unroll
-              for (int q = 0; q < NCOMP; ++q) {
-                if (WEIGHTED)
-                  atomicAdd(node + q * G::COMP, __float2int_rn(wxy * wzs[q][c]));
-                else
-                  atomicAdd(reinterpret_cast<unsigned*>(node + q * G::COMP), __float2uint_rn(wxy * wzs[q][c]));
+                for (int q = 0; q < NCOMP; ++q) {
+                  if (WEIGHTED)
+                    atomicAdd(node + q * G::COMP, __float2int_rn(wxy * wzs[q][c]));
+                  else
+                    atomicAdd(reinterpret_cast<unsigned*>(node + q * G::COMP), __float2uint_rn(wxy * wzs[q][c]));
+                }
               }
             }
-          }
+        }
+        if (last) {  // slot k is free: request the next item's record (its first batch)
+          const uint32_t ni = nbegin + (uint32_t)(k * BLOCK + tid);
+          if (ni < nend) load_rec<WEIGHTED>(r[k], bv, ni);
+        }
       }
-    }
+      if (last) break;
       b0 += CHUNK;
-      if (b0 >= iend) break;  // uniform
-      load_batch(b0, iend);   // dense tile: further batches of the same item
+      load_batch(b0, iend);  // dense tile: further batches of the same item
       load_weights(b0);
     }
     __syncthreads();
-    it = s_next[par];
+    const uint32_t nn = s_next[par];
     par ^= 1;
-    if (it < nitems) load_item(it);
+    WorkItem nnwi = nwi;
+    if (nn < nitems) nnwi = bv.items[nn];  // consumed after the flush
 
     // flush: vectorised global reductions along z (red.global.add.v4.f32), empty groups skipped; the
     // accumulators are zeroed on the way out.
@@ -434,9 +456,158 @@ __global__ void __launch_bounds__(BLOCK) k_scatter(BinView bv, typename T::Param
         }
       }
     }
-    __syncthreads();
+    if (NBUF == 1)
+      __syncthreads();  // the single buffer must be clean before the next deposit
+    else
+      s_acc = (s_acc == s_acc_all) ? s_acc_all + ACC : s_acc_all;
+    it = nxt;
+    wi = nwi;
+    nxt = nn;
+    nwi = nnwi;
   }
   if (tid == 0) sched_done(bv.sched);
+}
+
+// ---- K2, warp-private variant: unit weights, one field -------------------------------------------------
+// One WARP per work item, the accumulator tile private to the warp: there is no CTA barrier anywhere (in the
+// CTA-cooperative kernel above 35 % of the warp samples sat at the barrier between deposit and flush, ncu
+// round 1).  A lane deposits every 32nd record of the item (coalesced 512-byte record loads, WD records per lane
+// in flight, refilled as they are consumed, the next item's first records at the end), then the warp flushes its
+// tile.  Used where WS_WARPS accumulator tiles per CTA fit several CTAs on an SM (CIC); the cooperative kernel
+// serves the wider kernels, weights and vector fields.
+constexpr int WS_WARPS = 4;  // warps per CTA
+constexpr int WD = 8;        // records in flight per lane
+
+__device__ __forceinline__ uint32_t wsched_next(uint32_t* sched, uint32_t nwarps) {
+  return nwarps + atomicAdd(&sched[0], 1u);
+}
+__device__ __forceinline__ void wsched_done(uint32_t* sched, uint32_t nwarps) {
+  if (atomicAdd(&sched[1], 1u) == nwarps - 1u) {
+    sched[0] = 0u;
+    sched[1] = 0u;
+  }
+}
+
+template <class T>
+__global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, typename T::Params tp, int3 roll,
+                                                                   float* __restrict__ mesh) {
+  using G = Geo<T>;
+  constexpr int P = T::P;
+  constexpr int NG = G::NGROUP;
+  extern __shared__ __align__(16) int s_acc_all[];
+  const unsigned lane = threadIdx.x & 31u;
+  int* s_acc = s_acc_all + (threadIdx.x >> 5) * G::COMP;
+  const uint32_t nitems = *bv.nitems;
+  const uint32_t nwarps = gridDim.x * WS_WARPS;
+  const int m = bv.m;
+
+  for (int j = (int)lane; j < G::COMP / 4; j += 32) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
+  __syncwarp();
+
+  uint32_t it = blockIdx.x * WS_WARPS + (threadIdx.x >> 5), nxt = 0;
+  if (lane == 0) nxt = wsched_next(bv.sched, nwarps);
+  nxt = __shfl_sync(0xffffffffu, nxt, 0);
+  WorkItem wi, nwi;
+  wi.begin = wi.end = wi.txyz = nwi.begin = nwi.end = nwi.txyz = 0;
+  uint4 r[WD];
+#pragma unroll
+  for (int k = 0; k < WD; ++k) r[k] = make_uint4(0u, 0u, 0u, 0u);
+  if (it < nitems) {
+    wi = bv.items[it];
+#pragma unroll
+    for (int k = 0; k < WD; ++k) {
+      const uint32_t i = wi.begin + (uint32_t)(k * 32) + lane;
+      if (i < wi.end) load_rec<false>(r[k], bv, i);
+    }
+  }
+  if (nxt < nitems) nwi = bv.items[nxt];
+
+  while (it < nitems) {
+    uint32_t nn = 0;
+    if (lane == 0) nn = wsched_next(bv.sched, nwarps);  // item i+2; consumed after the deposit
+    const uint32_t n = wi.end - wi.begin;
+    const uint32_t iend = wi.end;
+    const TileOrigin o = tile_origin(wi);
+    const uint32_t nbegin = nwi.begin, nend = nxt < nitems ? nwi.end : nwi.begin;
+
+    // fixed-point scale: no node can receive more than n * WMAX3 (see k_scatter)
+    const float bound = (float)n * T::WMAX3;
+    int e = 0;
+    const float f = frexpf(bound, &e);
+    const int sexp = min(31, 31 - ((f == 0.5f) ? e - 1 : e));
+    const float scale = pow2i(sexp), inv_scale = pow2i(-sexp);
+
+    for (uint32_t b0 = wi.begin;; b0 += WD * 32) {
+      const bool last = b0 + WD * 32 >= iend;  // uniform
+#pragma unroll
+      for (int k = 0; k < WD; ++k) {
+        const uint32_t i = b0 + (uint32_t)(k * 32) + lane;
+        const uint4 rk = r[k];
+        const uint32_t pi = last ? nbegin + (uint32_t)(k * 32) + lane : i + (uint32_t)(WD * 32);
+        if (pi < (last ? nend : iend)) load_rec<false>(r[k], bv, pi);
+        if (i < iend) {
+          int sx, sy, sz;
+          float wx[P], wy[P], wz[P], dummy[P];
+          T::template axis<false>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dummy);
+          T::template axis<false>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dummy);
+          T::template axis<false>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dummy);
+          NodeCol nc[P];
+#pragma unroll
+          for (int c = 0; c < P; ++c) {
+            nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
+            wz[c] *= scale;
+          }
+#pragma unroll
+          for (int a = 0; a < P; ++a)
+#pragma unroll
+            for (int b = 0; b < P; ++b) {
+              const float wxy = wx[a] * wy[b];
+#pragma unroll
+              for (int c = 0; c < P; ++c)
+                atomicAdd(reinterpret_cast<unsigned*>(s_acc + ((a * G::SY + b) * nc[c].pitch + nc[c].base)),
+                          __float2uint_rn(wxy * wz[c]));
+            }
+        }
+      }
+      if (last) break;
+    }
+    __syncwarp();  // the lanes' deposits are visible to the flush below
+
+    nn = __shfl_sync(0xffffffffu, nn, 0);
+    WorkItem nnwi = nwi;
+    if (nn < nitems) nnwi = bv.items[nn];
+
+    // flush (as in k_scatter): red.global.add.v4.f32 per group of 4 nodes along z, empty groups skipped
+    const int bx = wrap_lo(o.x0 - G::HLO - roll.x, m), by = wrap_lo(o.y0 - G::HLO - roll.y, m);
+    const int bz = wrap_lo(o.z0 - G::ZLO - roll.z, m);
+    for (int j = (int)lane; j < NG; j += 32) {
+      int4* src = reinterpret_cast<int4*>(s_acc) + j;
+      const int4 v = *src;
+      if ((v.x | v.y | v.z | v.w) == 0) continue;
+      *src = make_int4(0, 0, 0, 0);
+      int row, zoff;
+      group_pos<G>(j, row, zoff);
+      const int sx = row / G::SY, sy = row - sx * G::SY;
+      const float4 fv = make_float4(__uint2float_rn((unsigned)v.x) * inv_scale, __uint2float_rn((unsigned)v.y) * inv_scale,
+                                    __uint2float_rn((unsigned)v.z) * inv_scale, __uint2float_rn((unsigned)v.w) * inv_scale);
+      const int gx = wrap_hi(bx + sx, m), gy = wrap_hi(by + sy, m), gz = wrap_hi(bz + zoff, m);
+      float* p = mesh + (size_t)(unsigned)(gx * m + gy) * (unsigned)m;
+      if ((gz & 3) == 0) {
+        red_add_v4(p + gz, fv);
+      } else {  // integer part of the shift not a multiple of 4: scalar reductions, each wrapped
+        atomicAdd(p + gz, fv.x);
+        atomicAdd(p + wrap_hi(gz + 1, m), fv.y);
+        atomicAdd(p + wrap_hi(gz + 2, m), fv.z);
+        atomicAdd(p + wrap_hi(gz + 3, m), fv.w);
+      }
+    }
+    __syncwarp();  // the tile is clean before the next deposit
+    it = nxt;
+    wi = nwi;
+    nxt = nn;
+    nwi = nnwi;
+  }
+  if (lane == 0) wsched_done(bv.sched, nwarps);
 }
 
 // ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) --------------------------------------
@@ -524,6 +695,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     fence_barrier_init();
     fence_proxy_async();
     if (manual >> 1) policy = l2_policy_evict_last();
+    s_next[0] = sched_next(bv.sched);  // the item after this CTA's first
   }
   __syncthreads();
 
@@ -532,9 +704,9 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     cy = wrap_lo(o.y0 - G::HLO - roll.y, m);
     cz = wrap_lo(o.z0 - G::ZLO - roll.z, m);
   };
-  auto issue = [&](uint32_t item, int stage) {  // thread 0
+  auto issue = [&](const WorkItem& w, int stage) {  // thread 0
     if (manual & 1) return;
-    const TileOrigin o = tile_origin(bv.items[item]);
+    const TileOrigin o = tile_origin(w);
     int cx, cy, cz;
     box_start(o, cx, cy, cz);
     mbar_expect_tx(&s_bar[stage], BOX_BYTES);
@@ -547,27 +719,32 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   };
 
   uint32_t phases = 0;  // bit s: parity the next wait on stage s uses
-  int stage = 0, par = 0;
-  uint32_t it = blockIdx.x;
-  if (tid == 0 && it < nitems) issue(it, 0);
-
-  while (it < nitems) {
-    if (tid == 0) {
-      const uint32_t next = sched_next(bv.sched);
-      s_next[par] = next;
-      if (STAGES == 2 && next < nitems) issue(next, stage ^ 1);
-    }
-    const WorkItem wi = bv.items[it];
-    const TileOrigin o = tile_origin(wi);
-    const float* s_val = s_base + stage * NCOMP * G::COMP;
-
-    // first batch of records: in flight while the box lands
-    uint4 r[KB];
+  int stage = 0, par = 1;
+  uint32_t it = blockIdx.x, nxt = s_next[0];
+  WorkItem wi, nwi;
+  wi.begin = wi.end = wi.txyz = nwi.begin = nwi.end = nwi.txyz = 0;
+  uint4 r[KB];  // records in flight: the slot a particle frees is refilled KB * BLOCK records ahead
+#pragma unroll
+  for (int k = 0; k < KB; ++k) r[k] = make_uint4(0u, 0u, 0u, 0u);
+  if (it < nitems) {
+    wi = bv.items[it];
+    if (tid == 0) issue(wi, 0);
 #pragma unroll
     for (int k = 0; k < KB; ++k) {
       const uint32_t i = wi.begin + (uint32_t)(k * BLOCK + tid);
-      if (i < wi.end) r[k] = load_rec(bv.rec + i);
+      if (i < wi.end) load_rec<true>(r[k], bv, i);
     }
+  }
+  if (nxt < nitems) nwi = bv.items[nxt];
+
+  while (it < nitems) {
+    if (tid == 0) {
+      s_next[par] = sched_next(bv.sched);  // item i+2
+      if (STAGES == 2 && nxt < nitems) issue(nwi, stage ^ 1);
+    }
+    const TileOrigin o = tile_origin(wi);
+    const float* s_val = s_base + stage * NCOMP * G::COMP;
+    const uint32_t nbegin = nwi.begin, nend = nxt < nitems ? nwi.end : nwi.begin;  // empty when there is no next item
 
     if (!(manual & 1)) {
       mbar_wait(&s_bar[stage], (phases >> stage) & 1u);
@@ -594,19 +771,16 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
       __syncthreads();
     }
 
-    for (uint32_t b0 = wi.begin; b0 < wi.end; b0 += KB * BLOCK) {
-      if (b0 != wi.begin) {
-#pragma unroll
-        for (int k = 0; k < KB; ++k) {
-          const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
-          if (i < wi.end) r[k] = load_rec(bv.rec + i);
-        }
-      }
+    for (uint32_t b0 = wi.begin;; b0 += KB * BLOCK) {  // at least once: the last pass requests the next item's records
+      const bool last = b0 + KB * BLOCK >= wi.end;  // uniform
 #pragma unroll
       for (int k = 0; k < KB; ++k) {
         const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
-        if (i >= wi.end) continue;
         const uint4 rk = r[k];
+        // refill the slot: the record one batch ahead, or (last batch) the next item's first batch
+        const uint32_t pi = last ? nbegin + (uint32_t)(k * BLOCK + tid) : i + (uint32_t)(KB * BLOCK);
+        if (pi < (last ? nend : wi.end)) load_rec<true>(r[k], bv, pi);
+        if (i >= wi.end) continue;
         int sx, sy, sz;
         float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
         T::template axis<GRAD>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
@@ -665,15 +839,22 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
           dst[2] = accumulate ? fmaf(alpha, gz, dst[2]) : alpha * gz;
         }
       }
+      if (last) break;
     }
     __syncthreads();  // every thread is done with this stage: it may be refilled
-    it = s_next[par];
+    const uint32_t nn = s_next[par];
     par ^= 1;
+    WorkItem nnwi = nwi;
+    if (nn < nitems) nnwi = bv.items[nn];
     if (STAGES == 2) {
       stage ^= 1;
-    } else if (tid == 0 && it < nitems) {
-      issue(it, 0);
+    } else if (tid == 0 && nxt < nitems) {
+      issue(nwi, 0);
     }
+    it = nxt;
+    wi = nwi;
+    nxt = nn;
+    nwi = nnwi;
   }
   if (tid == 0) sched_done(bv.sched);
 }
@@ -699,8 +880,10 @@ template <class T, int NCOMP, bool WEIGHTED>
 int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const float* wsrc, int wstride,
                 float* const mesh[], cudaStream_t st) {
   using G = Geo<T>;
-  const size_t smem = sizeof(int) * (size_t)NCOMP * G::COMP;
-  auto kern = k_scatter<T, NCOMP, WEIGHTED>;
+  constexpr size_t acc_bytes = sizeof(int) * (size_t)NCOMP * G::COMP;
+  constexpr int NBUF = 2 * acc_bytes <= 48 * 1024 ? 2 : 1;  // two accumulator tiles when they are cheap
+  const size_t smem = NBUF * acc_bytes;
+  auto kern = k_scatter<T, NCOMP, WEIGHTED, NBUF>;
   static int occ = 0;
   if (!occ) {
     PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -713,6 +896,28 @@ int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const f
   kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp,
                                                make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m)),
                                                wsrc, wstride, mp);
+  count_launch(c);
+  PM_CUDA(c, cudaGetLastError());
+  return PM_OK;
+}
+
+// Unit-weight, single-field scatter with warp-private tiles (k_scatter_warp).
+template <class T>
+int run_scatter_warp(Ctx* c, const typename T::Params& tp, const int roll[3], float* mesh, cudaStream_t st) {
+  using G = Geo<T>;
+  constexpr size_t smem = sizeof(int) * (size_t)WS_WARPS * G::COMP;
+  auto kern = k_scatter_warp<T>;
+  static int occ = 0;
+  if (!occ) {
+    PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    PM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WS_WARPS * 32, smem));
+    if (occ < 1) return fail(c, PM_ECUDA, "scatter kernel does not fit on an SM");
+  }
+  const int64_t bound = ((int64_t)c->ntiles + c->bin_n / ITEM_MAX + 1 + WS_WARPS - 1) / WS_WARPS;
+  const int64_t cap = (int64_t)c->num_sms * occ;
+  const int m = c->mg;
+  kern<<<(int)(bound < cap ? bound : cap), WS_WARPS * 32, smem, st>>>(
+      bin_view(c), tp, make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m)), mesh);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

@@ -11,7 +11,17 @@ static int scatter_os(Ctx* c, const ShiftSplit& sh, int ncomp, const float* wsrc
   typename T::Params tp;
   for (int a = 0; a < 3; ++a) tp.frac[a] = sh.frac[a];
   if (!wsrc) {  // unit weights: every component receives the same field
-    for (int a = 0; a < ncomp; ++a) PM_TRY((run_scatter<T, 1, false>(c, tp, sh.roll, nullptr, 0, mesh + a, st)));
+    // CIC: four warp-private accumulator tiles per CTA fit four CTAs on an SM -> the barrier-free kernel
+    static const bool coop = tune_flag("PMF_SCATTER_COOP", 0) != 0;  // A/B switch for measurements
+    for (int a = 0; a < ncomp; ++a) {
+      if constexpr (ORDER == 2) {
+        if (!coop) {
+          PM_TRY((run_scatter_warp<T>(c, tp, sh.roll, mesh[a], st)));
+          continue;
+        }
+      }
+      PM_TRY((run_scatter<T, 1, false>(c, tp, sh.roll, nullptr, 0, mesh + a, st)));
+    }
     return PM_OK;
   }
   if (ncomp == 3) return run_scatter<T, 3, true>(c, tp, sh.roll, wsrc, wstride, mesh, st);

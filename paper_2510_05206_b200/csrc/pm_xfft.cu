@@ -4,7 +4,8 @@
 // The 3-D transforms are split as (y,z) planes x lines.  cuFFT does the batched 2-D (y,z) transforms (library
 // call, "FFT"); this kernel then takes, for 8 neighbouring (y,z) columns at a time, the whole x line
 // into shared memory, runs the forward x-FFT, applies the Green's function / gradient symbols / deconvolution /
-// interlace combine of pm_kspace.cu (Tables 1-2) and runs the three inverse x-FFTs, so that
+// interlace combine of pm_kspace.cu (Tables 1-2) and runs the inverse x-FFTs (two of them: the y
+// and z gradient symbols are constant along x, so those two components share one inverse transform), so that
 // the spectrum is read once and the three force spectra are written once.  Unfused, the same work is five more
 // passes over the data: forward x pass (read + write), k-space kernel (read, 3 writes), three inverse x passes
 // (read + write each): 6.4 GB instead of 2.1 GB at 512^3.
@@ -197,7 +198,9 @@ __device__ __forceinline__ int xfft_freq(int p) {
 }
 
 struct XTabs {
-  const double *grad, *lap, *win, *pc, *ps;  // per-axis symbol tables of pm_kspace.cu
+  const double *grad, *lap, *win, *pc, *ps;  // per-axis symbol tables of pm_kspace.cu (column factors, once per thread)
+  const float4* sym;                         // the same along the line, fp32: {lap, win, grad, 0} per index
+  const float2* ph;                          // {pc, ps} per index
   const float2* tw;                          // e^{-2 pi i k / m}, k = 0 .. m-1
   int m, hz;
   int64_t ncol;                              // m * hz columns per x plane
@@ -239,14 +242,21 @@ __global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? 3 : 1) k_xfft_kspace(
   const float dyv = (float)t.grad[iy], dzv = (float)t.grad[iz];
   const double pcyz = t.pc[iy] * t.pc[iz] - t.ps[iy] * t.ps[iz], psyz = t.pc[iy] * t.ps[iz] + t.ps[iy] * t.pc[iz];
 
-  auto green_of = [&](int kx) -> float {  // coeff / (Lap * window); 0 at n = 0 and for dropped modes
-    const double den = (lyz + t.lap[kx]) * (wyz * t.win[kx]);
-    return den != 0.0 ? (float)(coeff_eff / den) : 0.0f;
+  // coeff / (Lap * window); 0 at n = 0 and for dropped modes.  The column part of the symbols is summed in fp64
+  // once per thread; along the line everything is fp32 (the result is an fp32 factor anyway; the fp64 adds,
+  // multiplies and the divide per mode were a quarter of the kernel's stall samples).
+  const float coeff_f = (float)coeff_eff, lyz_f = (float)lyz, wyz_f = (float)wyz;
+  const float pcyz_f = (float)pcyz, psyz_f = (float)psyz;
+  auto green_of = [&](int kx) -> float {
+    const float4 sy = __ldg(t.sym + kx);
+    const float den = (lyz_f + sy.x) * (wyz_f * sy.y);
+    return den != 0.0f ? __fdiv_rn(coeff_f, den) : 0.0f;
   };
   auto phase_of = [&](int kx) -> float2 {  // interlace phase e^{-ik.s} (real part only on Nyquist planes, R9)
-    return make_float2((float)(t.pc[kx] * pcyz - t.ps[kx] * psyz), (float)(t.pc[kx] * psyz + t.ps[kx] * pcyz));
+    const float2 e = __ldg(t.ph + kx);
+    return make_float2(e.x * pcyz_f - e.y * psyz_f, e.x * psyz_f + e.y * pcyz_f);
   };
-  auto grad_of = [&](int a, int kx) -> float { return a == 0 ? (float)t.grad[kx] : (a == 1 ? dyv : dzv); };
+  auto grad_of = [&](int a, int kx) -> float { return a == 0 ? __ldg(&t.sym[kx].z) : (a == 1 ? dyv : dzv); };
 
   // In every transform the last forward stage and the first inverse stage give a thread the same elements
   // (same radix, same sub-transform size), so s_a is only ever touched by the thread that owns the element.
@@ -265,32 +275,46 @@ __global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? 3 : 1) k_xfft_kspace(
       const float g = green_of(xfft_freq<N>(p));
       s_a[sidx(p, cc)] = make_float2(g * v.x, g * v.y);
     });
-#pragma unroll 1
-    for (int a = 0; a < 3; ++a) {
-      float2* dst = a == 0 ? out0 : (a == 1 ? out1 : out2);
-      xfft_line<N, true>(
-          s_w, t.tw, tid,
-          [&](int p, int cc) {  // -i D_a (re + i im) = D_a (im - i re)
-            const float dm = grad_of(a, xfft_freq<N>(p));
-            const float2 d = s_a[sidx(p, cc)];
-            return make_float2(dm * d.y, -dm * d.x);
-          },
-          gst(dst));
-    }
+    // x component: the gradient symbol varies along the line
+    xfft_line<N, true>(
+        s_w, t.tw, tid,
+        [&](int p, int cc) {  // -i D_x (re + i im) = D_x (im - i re)
+          const float dm = grad_of(0, xfft_freq<N>(p));
+          const float2 d = s_a[sidx(p, cc)];
+          return make_float2(dm * d.y, -dm * d.x);
+        },
+        gst(out0));
+    // y and z components: their gradient symbols are constant along x, so ONE inverse transform serves both
+    // (x-inverse of -i D_y A = -i D_y x-inverse of A); the factor is applied to the output.
+    xfft_line<N, true>(
+        s_w, t.tw, tid, [&](int p, int cc) { return s_a[sidx(p, cc)]; },
+        [&](int p, int, float2 v) {
+          if (live) {
+            out1[(size_t)p * plane + q] = make_float2(dyv * v.y, -dyv * v.x);
+            out2[(size_t)p * plane + q] = make_float2(dzv * v.y, -dzv * v.x);
+          }
+        });
   } else {
     const bool two = out1 != nullptr;
-#pragma unroll 1
-    for (int a = 0; a < 3; ++a) {
-      const float2* src = a == 0 ? in0 : (a == 1 ? in1 : in2);
-      xfft_line<N, false>(s_w, t.tw, tid, gld(src), [&](int p, int cc, float2 v) {
-        // conj(S_a) = +i D_a green:  q += i D_a (re + i im); green is applied on the way out
-        const float dm = grad_of(a, xfft_freq<N>(p));
-        float2 acc = a == 0 ? make_float2(0.f, 0.f) : s_a[sidx(p, cc)];
-        acc.x -= dm * v.y;
-        acc.y += dm * v.x;
-        s_a[sidx(p, cc)] = acc;
-      });
-    }
+    // conj(S_a) = +i D_a green:  q = i [D_x FFT_x(g_x) + FFT_x(D_y g_y + D_z g_z)]; green is applied on the way
+    // out.  D_y, D_z are constant along x, so the y and z cotangents share one forward transform.
+    xfft_line<N, false>(s_w, t.tw, tid, gld(in0), [&](int p, int cc, float2 v) {
+      const float dm = grad_of(0, xfft_freq<N>(p));
+      s_a[sidx(p, cc)] = make_float2(-dm * v.y, dm * v.x);
+    });
+    xfft_line<N, false>(
+        s_w, t.tw, tid,
+        [&](int p, int) {
+          if (!live) return make_float2(0.f, 0.f);
+          const float2 a = __ldcs(in1 + (size_t)p * plane + q), b = __ldcs(in2 + (size_t)p * plane + q);
+          return make_float2(dyv * a.x + dzv * b.x, dyv * a.y + dzv * b.y);
+        },
+        [&](int p, int cc, float2 v) {
+          float2 acc = s_a[sidx(p, cc)];
+          acc.x -= v.y;
+          acc.y += v.x;
+          s_a[sidx(p, cc)] = acc;
+        });
 #pragma unroll 1
     for (int o = 0; o < (two ? 2 : 1); ++o) {
       xfft_line<N, true>(
@@ -324,6 +348,25 @@ int xfft_init(Ctx* c) {  // twiddle table and the batched 2-D (y,z) cuFFT plans;
   }
   PM_CUDA(c, cudaMalloc((void**)&c->xtw, sizeof(float2) * (size_t)m));
   PM_CUDA(c, cudaMemcpy(c->xtw, tw.data(), sizeof(float2) * (size_t)m, cudaMemcpyHostToDevice));
+  {  // fp32 copies of the per-axis symbol tables, packed for one load per mode
+    std::vector<double> g(m), l(m), w(m), pc(m), ps(m);
+    const size_t nb = sizeof(double) * (size_t)m;
+    PM_CUDA(c, cudaMemcpy(g.data(), c->tab_grad, nb, cudaMemcpyDeviceToHost));
+    PM_CUDA(c, cudaMemcpy(l.data(), c->tab_lap, nb, cudaMemcpyDeviceToHost));
+    PM_CUDA(c, cudaMemcpy(w.data(), c->tab_win, nb, cudaMemcpyDeviceToHost));
+    PM_CUDA(c, cudaMemcpy(pc.data(), c->tab_cos, nb, cudaMemcpyDeviceToHost));
+    PM_CUDA(c, cudaMemcpy(ps.data(), c->tab_sin, nb, cudaMemcpyDeviceToHost));
+    std::vector<float4> sym(m);
+    std::vector<float2> ph(m);
+    for (int k = 0; k < m; ++k) {
+      sym[k] = make_float4((float)l[k], (float)w[k], (float)g[k], 0.f);
+      ph[k] = make_float2((float)pc[k], (float)ps[k]);
+    }
+    PM_CUDA(c, cudaMalloc((void**)&c->xsym, sizeof(float4) * (size_t)m));
+    PM_CUDA(c, cudaMemcpy(c->xsym, sym.data(), sizeof(float4) * (size_t)m, cudaMemcpyHostToDevice));
+    PM_CUDA(c, cudaMalloc((void**)&c->xph, sizeof(float2) * (size_t)m));
+    PM_CUDA(c, cudaMemcpy(c->xph, ph.data(), sizeof(float2) * (size_t)m, cudaMemcpyHostToDevice));
+  }
   int n2[2] = {m, m};
   size_t ws1 = 0, ws2 = 0;
   PM_CUFFT(c, cufftCreate(&c->plan2_r2c));
@@ -377,6 +420,8 @@ static int xfft_launch(Ctx* c, const float2* i0, const float2* i1, const float2*
   t.pc = c->tab_cos;
   t.ps = c->tab_sin;
   t.tw = c->xtw;
+  t.sym = c->xsym;
+  t.ph = c->xph;
   t.m = c->mg;
   t.hz = c->mg / 2 + 1;
   t.ncol = (int64_t)t.m * t.hz;

@@ -36,7 +36,8 @@ int spectra_to_force_meshes(Ctx* c, int ngrids, double coeff_eff, cudaStream_t s
 // a1: assignment of unit-mass particles onto the ctx meshes (interlace 1: also the half-cell shifted grid)
 int assign_ctx_meshes(Ctx* c, const ShiftSplit& sh, bool second_grid, cudaStream_t st) {
   stage_begin(c, PM_STAGE_ASSIGN, st);
-  PM_CUDA(c, cudaMemsetAsync(c->rho[0], 0, sizeof(float) * (size_t)c->G, st));
+  if (!c->zero_done) PM_CUDA(c, cudaMemsetAsync(c->rho[0], 0, sizeof(float) * (size_t)c->G, st));
+  c->zero_done = false;  // consumed: a second evaluation in the same call clears the mesh itself
   if (c->p.method == 0) {
     PM_TRY(launch_scatter(c, c->p.worder, sh, 1, nullptr, 0, &c->rho[0], st));
     if (second_grid) {
@@ -273,7 +274,12 @@ int pm_force(pm_ctx* ctx, const float* pos, int64_t N, float* force, void* strea
   cudaStream_t st = S(stream);
   reset_profile(c);
   stage_begin(c, PM_STAGE_BIN, st);
-  PM_TRY(ensure_bins(c, pos, N, st, false));
+  c->zero_done = false;
+  c->zero_req = c->rho[0];  // cleared by the histogram pass when it runs (pm_bin.cu, zero-fill rider)
+  c->zero_req_bytes = sizeof(float) * (size_t)c->G;
+  const int brc = ensure_bins(c, pos, N, st, false);
+  c->zero_req = nullptr;
+  PM_TRY(brc);
   stage_end(c, PM_STAGE_BIN, st);
   const ShiftSplit none = split_shift(c, nullptr);
   if (c->p.method == 0 && c->p.interlace == 2) {  // R1 mode 2: average of two complete evaluations
@@ -291,7 +297,12 @@ int pm_force_vjp(pm_ctx* ctx, const float* pos, int64_t N, const float* force_co
   cudaStream_t st = S(stream);
   reset_profile(c);
   stage_begin(c, PM_STAGE_BIN, st);
-  PM_TRY(ensure_bins(c, pos, N, st, false));
+  c->zero_done = false;
+  c->zero_req = c->rho[0];  // cleared by the histogram pass when it runs (pm_bin.cu, zero-fill rider)
+  c->zero_req_bytes = sizeof(float) * (size_t)c->G;
+  const int brc = ensure_bins(c, pos, N, st, false);
+  c->zero_req = nullptr;
+  PM_TRY(brc);
   stage_end(c, PM_STAGE_BIN, st);
   const ShiftSplit none = split_shift(c, nullptr);
   if (c->p.method == 0 && c->p.interlace == 2) {

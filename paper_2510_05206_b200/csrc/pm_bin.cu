@@ -140,15 +140,51 @@ __device__ __forceinline__ void claim_slots(uint32_t* __restrict__ counters, con
   }
 }
 
-// pass 1 (PERMUTE = false): tile histogram; pass 2 (PERMUTE = true): claim a slot, store the record.
+// MODE 0: tile histogram (first pass of the two-pass path).  MODE 1: second pass of the two-pass path: claim
+// a slot at tile_off[tile], store the record.  MODE 2: the single-pass ("bucketed") path: every tile owns a
+// bucket of `capt` record slots at rec[tile * capt]; a particle whose claim lands beyond the bucket goes to the
+// overflow list (record + tile id), which k_ov_permute sorts into rec[ov_base ...) afterwards.  No histogram
+// and no second read of the positions: 12N read + 16N written instead of 24N + 16N.
 // Positions are read as coalesced float4 (north_star "coalesced float4 position loads") and transposed
 // through a warp-private shared-memory strip so that lane l handles particles 32k + l, k = 0..3; the next
 // chunk's loads are in flight while the current one is processed.
-template <bool PERMUTE>
+struct Buckets {
+  uint32_t capt;       // slots per tile bucket
+  uint32_t* ov_count;  // overflow list length
+  uint4* ov_rec;       // overflow records (unsorted)
+  uint32_t* ov_tile;   // their tiles
+};
+
+template <int MODE>
+__device__ __forceinline__ void put_record(uint4* __restrict__ rec, const Buckets& bk, uint32_t tile, uint32_t toff,
+                                           uint32_t slot, bool valid, uint4 r) {
+  if (MODE == 1) {
+    if (valid) rec[toff + slot] = r;
+  } else if (MODE == 2) {
+    const bool ov = valid && slot >= bk.capt;
+    if (valid && !ov) rec[toff + slot] = r;
+    const unsigned ovm = __ballot_sync(0xffffffffu, ov);
+    if (ovm) {  // one atomic per warp for its overflowing lanes
+      const unsigned lane = threadIdx.x & 31u;
+      uint32_t base = 0;
+      if (lane == (unsigned)(__ffs(ovm) - 1)) base = atomicAdd(bk.ov_count, (uint32_t)__popc(ovm));
+      base = __shfl_sync(0xffffffffu, base, __ffs(ovm) - 1);
+      if (ov) {
+        const uint32_t j = base + (uint32_t)__popc(ovm & ((1u << lane) - 1u));
+        bk.ov_rec[j] = r;
+        bk.ov_tile[j] = tile;
+      }
+    }
+  }
+}
+
+template <int MODE>
 __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict__ pos, int64_t n, BinGeom g,
                                                         uint32_t* __restrict__ counters,
                                                         const uint32_t* __restrict__ tile_off,
-                                                        uint4* __restrict__ rec, int aligned) {
+                                                        uint4* __restrict__ rec, int aligned,
+                                                        float4* __restrict__ zfill, int64_t zn, int zq, Buckets bk) {
+  constexpr bool PERMUTE = MODE != 0;
   __shared__ __align__(16) float s_strip[BIN_BLOCK / 32][BIN_WARP_PART * 3];
   const unsigned lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
   float* s = s_strip[warp];
@@ -170,6 +206,12 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
       const float4* src = p4 + (ch + nwarps) * (BIN_WARP_PART * 3 / 4);
       a = __ldcs(src + lane), b = __ldcs(src + 32 + lane), c = __ldcs(src + 64 + lane);
     }
+    if (MODE != 1 && zfill) {  // zero-fill rider (see ensure_bins): chunk ch clears float4s [ch zq, (ch+1) zq)
+      for (int j = (int)lane; j < zq; j += 32) {
+        const int64_t idx = ch * zq + j;
+        if (idx < zn) __stcs(zfill + idx, make_float4(0.f, 0.f, 0.f, 0.f));
+      }
+    }
     uint32_t tile[4], slot[4], fx[4], fy[4], fz[4], toff[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -177,14 +219,15 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
       const float x = s[3 * j], y = s[3 * j + 1], z = s[3 * j + 2];
       fx[k] = fy[k] = fz[k] = 0;
       tile[k] = PERMUTE ? tile_and_local(x, y, z, g, fx[k], fy[k], fz[k]) : tile_only(x, y, z, g);
-      if (PERMUTE) toff[k] = __ldg(tile_off + tile[k]);
+      if (MODE == 1) toff[k] = __ldg(tile_off + tile[k]);
+      if (MODE == 2) toff[k] = tile[k] * bk.capt;
     }
     claim_slots<PERMUTE, 4>(counters, tile, slot);
     if (PERMUTE) {
 #pragma unroll
       for (int k = 0; k < 4; ++k)
-        rec[toff[k] + slot[k]] =
-            make_uint4(fx[k], fy[k], fz[k], (uint32_t)(ch * BIN_WARP_PART + 32 * k + (int)lane));
+        put_record<MODE>(rec, bk, tile[k], toff[k], slot[k], true,
+                         make_uint4(fx[k], fy[k], fz[k], (uint32_t)(ch * BIN_WARP_PART + 32 * k + (int)lane)));
     }
     __syncwarp();
   }
@@ -202,7 +245,25 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
       tile[0] = PERMUTE ? tile_and_local(x, y, z, g, fx, fy, fz) : tile_only(x, y, z, g);
     }
     claim_slots<PERMUTE, 1>(counters, tile, slot);
-    if (PERMUTE && valid) rec[tile_off[tile[0]] + slot[0]] = make_uint4(fx, fy, fz, (uint32_t)i);
+    if (PERMUTE) {
+      uint32_t toff = 0;
+      if (valid) toff = MODE == 1 ? tile_off[tile[0]] : tile[0] * bk.capt;
+      put_record<MODE>(rec, bk, tile[0], toff, slot[0], valid, make_uint4(fx, fy, fz, (uint32_t)i));
+    }
+  }
+}
+
+// Overflow of the single-pass path: sort the overflow list by tile into rec[ov_base + ov_off[tile] ...).
+__global__ void __launch_bounds__(256) k_ov_permute(const uint32_t* __restrict__ ov_count,
+                                                    const uint4* __restrict__ ov_rec,
+                                                    const uint32_t* __restrict__ ov_tile,
+                                                    const uint32_t* __restrict__ ov_off, uint32_t* __restrict__ ov_cur,
+                                                    uint4* __restrict__ rec, uint32_t ov_base) {
+  const uint32_t n = *ov_count;
+  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+    const uint32_t t = ov_tile[j];
+    const uint32_t slot = atomicAdd(&ov_cur[t], 1u);
+    rec[ov_base + ov_off[t] + slot] = ov_rec[j];
   }
 }
 
@@ -210,6 +271,13 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
 constexpr int SCAN_T = 1024, SCAN_E = 4, SCAN_B = SCAN_T * SCAN_E;
 
 __device__ __forceinline__ uint32_t nchunks_of(uint32_t cnt) { return (cnt + ITEM_MAX - 1) / ITEM_MAX; }
+// What the scan sums per tile.  Two-pass path (capt = 0): (particles, work items).  Single-pass path: (overflow
+// particles, work items of the bucket + work items of the overflow segment).
+__device__ __forceinline__ uint2 scan_pair(uint32_t cnt, uint32_t capt) {
+  if (capt == 0) return make_uint2(cnt, nchunks_of(cnt));
+  const uint32_t ov = cnt > capt ? cnt - capt : 0u;
+  return make_uint2(ov, nchunks_of(cnt - ov) + nchunks_of(ov));
+}
 
 __device__ uint2 block_exclusive_scan(uint2 v, uint2* total) {  // blockDim.x == SCAN_T
   __shared__ uint2 wsum[32];
@@ -240,13 +308,13 @@ __device__ uint2 block_exclusive_scan(uint2 v, uint2* total) {  // blockDim.x ==
 }
 
 __global__ void __launch_bounds__(SCAN_T) k_scan_reduce(const uint32_t* __restrict__ cnt, int n,
-                                                        uint2* __restrict__ partial) {
+                                                        uint2* __restrict__ partial, uint32_t capt) {
   __shared__ uint2 tot;
   uint2 s = make_uint2(0, 0);
   const int base = blockIdx.x * SCAN_B + threadIdx.x * SCAN_E;
 #pragma unroll
   for (int e = 0; e < SCAN_E; ++e)
-    if (base + e < n) { const uint32_t c = cnt[base + e]; s.x += c; s.y += nchunks_of(c); }
+    if (base + e < n) { const uint2 v = scan_pair(cnt[base + e], capt); s.x += v.x; s.y += v.y; }
   block_exclusive_scan(s, &tot);
   if (threadIdx.x == 0) partial[blockIdx.x] = tot;
 }
@@ -276,15 +344,15 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_partials(uint2* __restrict__ pa
 __global__ void __launch_bounds__(SCAN_T) k_scan_final(uint32_t* __restrict__ cnt, int n,
                                                        const uint2* __restrict__ partial,
                                                        uint32_t* __restrict__ tile_off,
-                                                       uint32_t* __restrict__ item_off) {
+                                                       uint32_t* __restrict__ item_off, uint32_t capt) {
   const int base = blockIdx.x * SCAN_B + threadIdx.x * SCAN_E;
-  uint32_t c[SCAN_E];
+  uint2 c[SCAN_E];
   uint2 s = make_uint2(0, 0);
 #pragma unroll
   for (int e = 0; e < SCAN_E; ++e) {
-    c[e] = base + e < n ? cnt[base + e] : 0u;
-    s.x += c[e];
-    s.y += nchunks_of(c[e]);
+    c[e] = base + e < n ? scan_pair(cnt[base + e], capt) : make_uint2(0u, 0u);
+    s.x += c[e].x;
+    s.y += c[e].y;
   }
   uint2 ex = block_exclusive_scan(s, nullptr);
   const uint2 p = partial[blockIdx.x];
@@ -295,9 +363,9 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_final(uint32_t* __restrict__ cn
     if (base + e < n) {
       tile_off[base + e] = ex.x;
       item_off[base + e] = ex.y;
-      ex.x += c[e];
-      ex.y += nchunks_of(c[e]);
-      cnt[base + e] = 0u;  // becomes the cursor of pass 2
+      ex.x += c[e].x;
+      ex.y += c[e].y;
+      if (capt == 0) cnt[base + e] = 0u;  // becomes the cursor of pass 2 (the single-pass path keeps the counts)
     }
 }
 
@@ -324,6 +392,40 @@ __global__ void __launch_bounds__(256) k_items(const uint32_t* __restrict__ tile
     w.end = min(w.begin + per, e);
     w.txyz = txyz;
     items[it++] = w;
+  }
+}
+
+// Work items of the single-pass path: the tile's bucket rec[t capt, + min(cnt, capt)) and, if it overflowed,
+// its overflow segment rec[ov_base + ov_off[t], + cnt - capt).
+__global__ void __launch_bounds__(256) k_items_bucketed(const uint32_t* __restrict__ cnt,
+                                                        const uint32_t* __restrict__ ov_off,
+                                                        const uint32_t* __restrict__ item_off, int ntiles, int nty,
+                                                        int ntz, int xbl, uint32_t capt, uint32_t ov_base,
+                                                        WorkItem* __restrict__ items) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= ntiles) return;
+  const uint32_t c = cnt[t];
+  const uint32_t ov = c > capt ? c - capt : 0u;
+  uint32_t it = item_off[t];
+  const int tz = t % ntz;
+  int r = t / ntz;
+  const int xl = r & ((1 << xbl) - 1);
+  r >>= xbl;
+  const int ty = r % nty, tx = ((r / nty) << xbl) | xl;
+  const uint32_t txyz = (uint32_t)tx | ((uint32_t)ty << 10) | ((uint32_t)tz << 20);
+  for (int seg = 0; seg < 2; ++seg) {
+    const uint32_t b = seg == 0 ? (uint32_t)t * capt : ov_base + ov_off[t];
+    const uint32_t e = b + (seg == 0 ? c - ov : ov);
+    const uint32_t k = nchunks_of(e - b);
+    const uint32_t per = k ? (e - b + k - 1) / k : 0;
+    for (uint32_t j = 0; j < k; ++j) {
+      WorkItem w;
+      w.tile = (uint32_t)t;
+      w.begin = min(b + j * per, e);
+      w.end = min(w.begin + per, e);
+      w.txyz = txyz;
+      items[it++] = w;
+    }
   }
 }
 
@@ -368,13 +470,50 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   int grid0 = grid;  // the histogram pass needs fewer registers: its own residency
   if (grid > c->num_sms * c->bin_occ) grid = c->num_sms * c->bin_occ;
   if (grid0 > c->num_sms * c->bin_occ0) grid0 = c->num_sms * c->bin_occ0;
-  if (N > 0) k_bin_pass<false><<<grid0, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, nullptr, aligned);
-  k_scan_reduce<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial);
-  k_scan_partials<<<1, SCAN_T, 0, st>>>(partial, nb, c->tile_off, c->item_off, nt, c->nitems);
-  k_scan_final<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, c->tile_off, c->item_off);
-  if (N > 0) k_bin_pass<true><<<grid, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, c->tile_off, c->rec, aligned);
-  k_items<<<(nt + 255) / 256, 256, 0, st>>>(c->tile_off, c->item_off, nt, c->nty, c->ntz, c->xbl, c->items);
-  count_launch(c, N > 0 ? 6 : 4);
+  // Zero-fill rider: the first pass over the positions also clears the assignment mesh pm_force needs next
+  // (one 16-byte store per lane and iteration at G = N), which saves the separate cudaMemset pass and its
+  // launch; the binning passes run at 40-80 % of the HBM roofline, so the stores fit beside their traffic.
+  float4* zfill = nullptr;
+  int64_t zn = 0, nchunk = aligned ? N / BIN_WARP_PART : 0;
+  int zq = 0;
+  if (c->zero_req && nchunk > 0 && (c->zero_req_bytes & 15u) == 0 &&
+      (int64_t)(c->zero_req_bytes / 16) <= nchunk * 4096) {
+    zfill = reinterpret_cast<float4*>(c->zero_req);
+    zn = (int64_t)(c->zero_req_bytes / 16);
+    zq = (int)((zn + nchunk - 1) / nchunk);
+    c->zero_done = true;
+  }
+  c->zero_req = nullptr;
+  Buckets bk;
+  bk.capt = c->bin_capt;
+  bk.ov_count = c->ov_count;
+  bk.ov_rec = c->ov_rec;
+  bk.ov_tile = c->ov_tile;
+  if (c->bin_capt) {
+    // single pass: bucketed permute, scan of the overflow counts, work items, overflow sort
+    PM_CUDA(c, cudaMemsetAsync(c->ov_count, 0, sizeof(uint32_t), st));
+    PM_CUDA(c, cudaMemsetAsync(c->ov_cur, 0, sizeof(uint32_t) * (size_t)nt, st));
+    if (N > 0)
+      k_bin_pass<2><<<grid, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, c->rec, aligned, zfill, zn, zq, bk);
+    k_scan_reduce<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, bk.capt);
+    k_scan_partials<<<1, SCAN_T, 0, st>>>(partial, nb, c->tile_off, c->item_off, nt, c->nitems);
+    k_scan_final<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, c->tile_off, c->item_off, bk.capt);
+    k_items_bucketed<<<(nt + 255) / 256, 256, 0, st>>>(c->tile_cnt, c->tile_off, c->item_off, nt, c->nty, c->ntz,
+                                                       c->xbl, bk.capt, c->ov_base, c->items);
+    k_ov_permute<<<c->num_sms * 4, 256, 0, st>>>(c->ov_count, c->ov_rec, c->ov_tile, c->tile_off, c->ov_cur, c->rec,
+                                                 c->ov_base);
+    count_launch(c, N > 0 ? 6 : 5);
+  } else {
+    if (N > 0)
+      k_bin_pass<0><<<grid0, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, nullptr, nullptr, aligned, zfill, zn, zq, bk);
+    k_scan_reduce<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, 0u);
+    k_scan_partials<<<1, SCAN_T, 0, st>>>(partial, nb, c->tile_off, c->item_off, nt, c->nitems);
+    k_scan_final<<<nb, SCAN_T, 0, st>>>(c->tile_cnt, nt, partial, c->tile_off, c->item_off, 0u);
+    if (N > 0)
+      k_bin_pass<1><<<grid, BIN_BLOCK, 0, st>>>(pos, N, g, c->tile_cnt, c->tile_off, c->rec, aligned, nullptr, 0, 0, bk);
+    k_items<<<(nt + 255) / 256, 256, 0, st>>>(c->tile_off, c->item_off, nt, c->nty, c->ntz, c->xbl, c->items);
+    count_launch(c, N > 0 ? 6 : 4);
+  }
   PM_CUDA(c, cudaGetLastError());
   c->bin_valid = true;
   c->bin_pos = pos;
@@ -385,10 +524,14 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
 
 int bin_occupancy(int pass) {
   int o = 0;
-  if (pass == 0)
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_bin_pass<false>, BIN_BLOCK, 0);
-  else
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_bin_pass<true>, BIN_BLOCK, 0);
+  if (pass == 0) {
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, k_bin_pass<0>, BIN_BLOCK, 0);
+  } else {
+    int a = 0, b = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, k_bin_pass<1>, BIN_BLOCK, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, k_bin_pass<2>, BIN_BLOCK, 0);
+    o = a < b ? a : b;
+  }
   return o < 1 ? 1 : o;
 }
 

@@ -244,9 +244,24 @@ static int build(Ctx* c) {
 
   // binning workspace
   c->cap = p.max_particles;
-  c->max_items = (int64_t)c->ntiles + c->cap / ITEM_MAX + 2;
+  c->max_items = 2 * (int64_t)c->ntiles + c->cap / ITEM_MAX + 2;
+  {  // single-pass binning: a bucket of twice the mean tile load per tile, overflow sorted behind the buckets
+    const char* e = getenv("PMF_BIN_TWOPASS");
+    const int64_t mean = (c->cap + c->ntiles - 1) / c->ntiles;
+    int64_t capt = (2 * mean + 31) / 32 * 32;
+    if (capt < 64) capt = 64;
+    const int64_t total = (int64_t)c->ntiles * capt + c->cap;
+    c->bin_capt = ((e && atoi(e) != 0) || total >= (int64_t)0xffffffff) ? 0u : (uint32_t)capt;
+    c->ov_base = (uint32_t)((int64_t)c->ntiles * c->bin_capt);
+  }
   const int scan_blocks = (c->ntiles + 4095) / 4096;
-  PM_CUDA(c, cudaMalloc((void**)&c->rec, sizeof(uint4) * (size_t)c->cap));
+  PM_CUDA(c, cudaMalloc((void**)&c->rec, sizeof(uint4) * ((size_t)c->ov_base + (size_t)c->cap)));
+  if (c->bin_capt) {
+    PM_CUDA(c, cudaMalloc((void**)&c->ov_count, sizeof(uint32_t)));
+    PM_CUDA(c, cudaMalloc((void**)&c->ov_rec, sizeof(uint4) * (size_t)(c->cap > 0 ? c->cap : 1)));
+    PM_CUDA(c, cudaMalloc((void**)&c->ov_tile, sizeof(uint32_t) * (size_t)(c->cap > 0 ? c->cap : 1)));
+    PM_CUDA(c, cudaMalloc((void**)&c->ov_cur, sizeof(uint32_t) * (size_t)c->ntiles));
+  }
   PM_CUDA(c, cudaMalloc((void**)&c->tile_cnt, sizeof(uint32_t) * (size_t)c->ntiles));
   PM_CUDA(c, cudaMalloc((void**)&c->tile_off, sizeof(uint32_t) * (size_t)(c->ntiles + 1)));
   PM_CUDA(c, cudaMalloc((void**)&c->item_off, sizeof(uint32_t) * (size_t)(c->ntiles + 1)));
@@ -309,7 +324,8 @@ static void teardown(Ctx* c) {
   void* ptrs[] = {c->tab_grad, c->tab_lap, c->tab_win, c->tab_cos, c->tab_sin, c->rec, c->tile_cnt,
                   c->tile_off, c->item_off, c->scan_tmp, c->items, c->nitems, c->sched, c->fft_work, c->rho[0],
                   c->rho[1], c->dhat[0], c->dhat[1], c->ghat[0], c->ghat[1], c->ghat[2], c->g[0],
-                  c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->xtw, c->xsym, c->xph, c->host_pos_dev,
+                  c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->xtw, c->xsym, c->xph, c->ov_count, c->ov_rec, c->ov_tile, c->ov_cur,
+                  c->host_pos_dev,
                   c->host_force_dev};
   for (void* q : ptrs)
     if (q) cudaFree(q);

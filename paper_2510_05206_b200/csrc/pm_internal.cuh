@@ -95,6 +95,10 @@ struct Ctx {
   int64_t Gh;    // mg^2 (mg/2+1)
   int ntx, nty, ntz, ntiles, xbl;
   int bin_occ0, bin_occ;  // resident CTAs per SM of the two binning passes
+  // zero-fill rider of the histogram pass (pm_bin.cu): pm_force asks ensure_bins to clear its assignment mesh
+  void* zero_req;
+  size_t zero_req_bytes;
+  bool zero_done;  // rho[0] was cleared by the binning pass of this call
   int nufft_w;
   double nufft_beta;
 
@@ -108,6 +112,12 @@ struct Ctx {
   // binning workspace
   int64_t cap;
   uint4* rec;
+  uint32_t bin_capt;    // slots per tile bucket of the single-pass binning; 0 = two-pass (histogram + permute)
+  uint32_t ov_base;     // first overflow record in rec: ntiles * bin_capt
+  uint32_t* ov_count;   // [1] overflow list length
+  uint4* ov_rec;        // [cap] overflow records, unsorted
+  uint32_t* ov_tile;    // [cap] their tiles
+  uint32_t* ov_cur;     // [ntiles] cursor of the overflow sort
   uint32_t* tile_cnt;   // [ntiles]   histogram, then reused as cursor
   uint32_t* tile_off;   // [ntiles+1]
   uint32_t* item_off;   // [ntiles+1]

@@ -488,7 +488,7 @@ __device__ __forceinline__ void wsched_done(uint32_t* sched, uint32_t nwarps) {
   }
 }
 
-template <class T>
+template <class T, bool FASTCIC>
 __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, typename T::Params tp, int3 roll,
                                                                    float* __restrict__ mesh) {
   using G = Geo<T>;
@@ -510,6 +510,7 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
   WorkItem wi, nwi;
   wi.begin = wi.end = wi.txyz = nwi.begin = nwi.end = nwi.txyz = 0;
   uint4 r[WD];
+  uint32_t keep = 0;  // xor of the records' .w: see the deposit loop
 #pragma unroll
   for (int k = 0; k < WD; ++k) r[k] = make_uint4(0u, 0u, 0u, 0u);
   if (it < nitems) {
@@ -543,9 +544,50 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
       for (int k = 0; k < WD; ++k) {
         const uint32_t i = b0 + (uint32_t)(k * 32) + lane;
         const uint4 rk = r[k];
+        // Keep the unused .w (original index) of the record LIVE until here (one LOP3 per record).  Otherwise
+        // ptxas reuses its register as scratch while the next 128-bit record load into r[k] is still in flight,
+        // and every such write waits for the load to land (write-after-write on the load's destination): ncu
+        // showed 66 % of the stall samples on the first instruction after each prefetch, 1.24 ms instead of
+        // 0.74 ms.  (An empty asm does not do it: it leaves no use in the PTX that ptxas sees.)
+        keep ^= rk.w;
         const uint32_t pi = last ? nbegin + (uint32_t)(k * 32) + lane : i + (uint32_t)(WD * 32);
         if (pi < (last ? nend : iend)) load_rec<false>(r[k], bv, pi);
         if (i < iend) {
+          if constexpr (FASTCIC && P == 2 && !T::SHIFT && G::ZLO == 0) {
+            // Unshifted CIC (the headline assign): the first z node is always in the MAIN plane (sz < TZ by the
+            // binning), so the four rows of a z node are ONE base address plus compile-time offsets; only
+            // sz = TZ - 1 sends the second z node to the HALO plane (a branch, not per-node selects).  The
+            // generic addressing below spent ~20 of its 72 instructions per particle on pitch/base selects
+            // and the kernel is issue-bound (ncu: 70 % issue active).
+            constexpr float INV = 1.0f / (float)REC_ONE;
+            const float tx = (float)(rk.x & REC_MASK) * INV, ty = (float)(rk.y & REC_MASK) * INV;
+            const float tzs = (float)(rk.z & REC_MASK) * (INV * scale);
+            const int sx = (int)(rk.x >> REC_FRAC) - REC_BIAS, sy = (int)(rk.y >> REC_FRAC) - REC_BIAS;
+            const int sz = (int)(rk.z >> REC_FRAC) - REC_BIAS;
+            const int row0 = sx * G::SY + sy;
+            const float ox = 1.0f - tx, oy = 1.0f - ty, ozs = scale - tzs;
+            const float w00 = ox * oy, w01 = ox * ty, w10 = tx * oy, w11 = tx * ty;
+            unsigned* p0 = reinterpret_cast<unsigned*>(s_acc) + (row0 * TZ + sz);
+            atomicAdd(p0, __float2uint_rn(w00 * ozs));
+            atomicAdd(p0 + TZ, __float2uint_rn(w01 * ozs));
+            atomicAdd(p0 + G::SY * TZ, __float2uint_rn(w10 * ozs));
+            atomicAdd(p0 + (G::SY + 1) * TZ, __float2uint_rn(w11 * ozs));
+            const unsigned u00 = __float2uint_rn(w00 * tzs), u01 = __float2uint_rn(w01 * tzs);
+            const unsigned u10 = __float2uint_rn(w10 * tzs), u11 = __float2uint_rn(w11 * tzs);
+            if (sz < TZ - 1) {
+              atomicAdd(p0 + 1, u00);
+              atomicAdd(p0 + TZ + 1, u01);
+              atomicAdd(p0 + G::SY * TZ + 1, u10);
+              atomicAdd(p0 + (G::SY + 1) * TZ + 1, u11);
+            } else {
+              unsigned* ph = reinterpret_cast<unsigned*>(s_acc) + (G::MAIN + row0 * G::HZ);
+              atomicAdd(ph, u00);
+              atomicAdd(ph + G::HZ, u01);
+              atomicAdd(ph + G::SY * G::HZ, u10);
+              atomicAdd(ph + (G::SY + 1) * G::HZ, u11);
+            }
+            continue;
+          }
           int sx, sy, sz;
           float wx[P], wy[P], wz[P], dummy[P];
           T::template axis<false>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dummy);
@@ -608,6 +650,7 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
     nwi = nnwi;
   }
   if (lane == 0) wsched_done(bv.sched, nwarps);
+  if (keep == 0x9e3779b9u && nitems == 0xffffffffu) mesh[0] = 0.f;  // never true: gives `keep` a consumer
 }
 
 // ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) --------------------------------------
@@ -906,7 +949,8 @@ template <class T>
 int run_scatter_warp(Ctx* c, const typename T::Params& tp, const int roll[3], float* mesh, cudaStream_t st) {
   using G = Geo<T>;
   constexpr size_t smem = sizeof(int) * (size_t)WS_WARPS * G::COMP;
-  auto kern = k_scatter_warp<T>;
+  static const bool fast = tune_flag("PMF_SCATTER_FASTCIC", 1) != 0;  // A/B switch for measurements
+  auto kern = fast ? k_scatter_warp<T, true> : k_scatter_warp<T, false>;
   static int occ = 0;
   if (!occ) {
     PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

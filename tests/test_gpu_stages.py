@@ -218,6 +218,32 @@ def test_edge_cases(pm):
     pm.pm_destroy(ctx)
 
 
+def test_bucket_overflow_of_single_pass_binning(pm):
+    """Half of the particles inside two tiles of a 64^3 mesh (128 tiles, bucket = twice the mean load): their
+    records overflow the tile buckets and take the overflow-sort path of the binning; assign and interp must
+    still match the oracle, and the forces must come back in caller order."""
+    m, box, n = 64, 64.0, 60000
+    rng = np.random.default_rng(11)
+    pu = rng.random((n // 2, 3)) * box
+    pa = rng.random((n // 4, 3)) * np.array([7.9, 7.9, 31.9]) + np.array([8.0, 16.0, 32.0])
+    pb = rng.random((n - n // 2 - n // 4, 3)) * np.array([7.9, 7.9, 31.9]) + np.array([56.0, 56.0, 0.0])
+    pos = np.concatenate([pu, pa, pb]).astype(np.float32)
+    pos = pos[rng.permutation(n)]
+    for worder in (2, 3):
+        ctx = pm.pm_create(pm.PMParams(m=m, box=box, max_particles=n, worder=worder))
+        mesh = torch.zeros(m, m, m, device="cuda")
+        pm.pm_assign(ctx, dev(pos), None, mesh)
+        ref = po.scatter(pos, m, box, worder)
+        assert rel_l2(mesh.cpu().numpy(), ref) <= 1e-6
+        assert abs(float(mesh.sum().cpu()) - n) <= 1e-4 * n
+        f = gen.random_mesh(m, 5, 3)
+        out = torch.empty(n, 3, device="cuda")
+        pm.pm_interp(ctx, [dev(f[a]) for a in range(3)], dev(pos), out)
+        refg = np.stack([po.gather(f[a], pos, box, worder) for a in range(3)], axis=1)
+        assert rel_l2(out.cpu().numpy(), refg) <= 1e-6
+        pm.pm_destroy(ctx)
+
+
 def test_errors_are_reported(pm):
     with pytest.raises(pm.PMError):
         pm.pm_create(pm.PMParams(m=30, box=1.0, max_particles=10))  # m not a multiple of 4

@@ -48,7 +48,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static EncodeTiledFn g_encode_tiled = nullptr;
 
-int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMap* out) {
+int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, bool swizzle128, CUtensorMap* out) {
   if (!g_encode_tiled) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -64,7 +64,8 @@ int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMa
   const cuuint32_t box[3] = {(cuuint32_t)sz, (cuuint32_t)sy, (cuuint32_t)sx};
   const cuuint32_t estr[3] = {1, 1, 1};
   const CUresult r = g_encode_tiled(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides,
-                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                    swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                                     (getenv("PMF_TMA_PROMO") ? (CUtensorMapL2promotion)atoi(getenv("PMF_TMA_PROMO")) : CU_TENSOR_MAP_L2_PROMOTION_L2_128B), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(c, PM_ECUDA, "cuTensorMapEncodeTiled failed: CUresult %d (box %d x %d x %d)", (int)r, sx, sy, sz);
   return PM_OK;

@@ -210,7 +210,8 @@ inline GatherArgs gather_values(int ncomp, const float* const* mesh, float* out,
 int launch_gather(Ctx* c, int order, const ShiftSplit& sh, const GatherArgs& a, cudaStream_t st);
 // Tensor map of a dense fp32 [m][m][m] mesh (m = c->mg) with a box of sx * sy * sz elements, no swizzle,
 // out-of-bounds elements zero-filled.  base must be 16-byte aligned (PM_EINVAL otherwise).
-int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMap* out);
+// swizzle128: the box rows (sz * 4 = 128 bytes) land in shared memory with TMA's 128-byte swizzle
+int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, bool swizzle128, CUtensorMap* out);
 
 // NUFFT spreading / interpolation with the ES kernel (same conventions).
 int launch_es_scatter(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[],

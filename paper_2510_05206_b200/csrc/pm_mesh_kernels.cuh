@@ -126,7 +126,7 @@ struct Geo {
   static constexpr int HZ = ZLO + (HHI + 3) / 4 * 4;                 // halo columns per row
   static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, NROW = SX * SY;
   static constexpr int MAIN = NROW * TZ, HAL = NROW * HZ;            // words per component
-  static constexpr int COMP = (MAIN + HAL + 31) / 32 * 32;           // component block (128-byte multiple)
+  static constexpr int COMP = (MAIN + HAL + 255) / 256 * 256;        // component block (1024-byte multiple: TMA swizzle atom)
   static constexpr int NGM = NROW * (TZ / 4), NGH = NROW * (HZ / 4); // float4 groups per component
   static constexpr int NGROUP = NGM + NGH;
   static_assert(TZ == 32, "the main plane's row pitch must be 32 words");
@@ -213,7 +213,16 @@ __device__ __forceinline__ uint32_t apply_shift(uint32_t rec, uint32_t frac) {
 // consecutive tiles: the halo planes two neighbouring tiles share are touched close together in time and
 // are served from L2.  (A static stride lets CTAs drift apart: ncu showed the TMA halo reads of the gather
 // all going to DRAM.)  The last CTA to finish zeroes both counters for the next launch on the stream.
-__device__ __forceinline__ uint32_t sched_next(uint32_t* sched) { return gridDim.x + atomicAdd(&sched[0], 1u); }
+// The counter is bumped with a raw atom.global.add: nvcc turns atomicAdd() under a lane-dependent branch into
+// a warp-aggregated sequence whose broadcast SHFL consumes the result AT ONCE, which exposes the contended
+// counter's whole round trip once per item (ncu: 18-20 % of the scatter's stall samples on that SHFL).  With the
+// raw instruction the result is first touched where the caller reads it, one work item later.
+__device__ __forceinline__ uint32_t atom_inc_raw(uint32_t* p) {
+  uint32_t r;
+  asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(r) : "l"(p) : "memory");
+  return r;
+}
+__device__ __forceinline__ uint32_t sched_next(uint32_t* sched) { return gridDim.x + atom_inc_raw(&sched[0]); }
 __device__ __forceinline__ void sched_done(uint32_t* sched) {
   if (atomicAdd(&sched[1], 1u) == gridDim.x - 1u) {
     sched[0] = 0u;
@@ -294,7 +303,10 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>())
   }
   if (nxt < nitems) nwi = bv.items[nxt];
   while (it < nitems) {
-    if (tid == 0) s_next[par] = sched_next(bv.sched);  // item i+2
+    // item i+2: the atomic is issued now and its result is only touched right before the barrier below (stored
+    // at once, thread 0 would wait ~microseconds for the contended counter with the whole CTA behind it)
+    uint32_t fetched = 0;
+    if (tid == 0) fetched = sched_next(bv.sched);
     const uint32_t n = wi.end - wi.begin;
     const uint32_t ibegin = wi.begin, iend = wi.end;
     const TileOrigin o = tile_origin(wi);
@@ -412,6 +424,7 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>())
       load_batch(b0, iend);  // dense tile: further batches of the same item
       load_weights(b0);
     }
+    if (tid == 0) s_next[par] = fetched;
     __syncthreads();
     const uint32_t nn = s_next[par];
     par ^= 1;
@@ -476,10 +489,10 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>())
 // tile.  Used where WS_WARPS accumulator tiles per CTA fit several CTAs on an SM (CIC); the cooperative kernel
 // serves the wider kernels, weights and vector fields.
 constexpr int WS_WARPS = 4;  // warps per CTA
-constexpr int WD = 8;        // records in flight per lane
+constexpr int WD = 10;       // records in flight per lane (128 registers per thread at 4 CTAs of 128 threads)
 
 __device__ __forceinline__ uint32_t wsched_next(uint32_t* sched, uint32_t nwarps) {
-  return nwarps + atomicAdd(&sched[0], 1u);
+  return nwarps + atom_inc_raw(&sched[0]);
 }
 __device__ __forceinline__ void wsched_done(uint32_t* sched, uint32_t nwarps) {
   if (atomicAdd(&sched[1], 1u) == nwarps - 1u) {
@@ -495,6 +508,7 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
   constexpr int P = T::P;
   constexpr int NG = G::NGROUP;
   extern __shared__ __align__(16) int s_acc_all[];
+  __shared__ volatile uint32_t s_mail[WS_WARPS];
   const unsigned lane = threadIdx.x & 31u;
   int* s_acc = s_acc_all + (threadIdx.x >> 5) * G::COMP;
   const uint32_t nitems = *bv.nitems;
@@ -613,9 +627,12 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
       }
       if (last) break;
     }
-    __syncwarp();  // the lanes' deposits are visible to the flush below
-
-    nn = __shfl_sync(0xffffffffu, nn, 0);
+    // The counter's value travels through a shared-memory mailbox, not a shuffle: ptxas hoisted the shuffle to
+    // right behind the atomic and the warp sat out the contended counter's round trip once per item (ncu: 18 %
+    // of the stall samples on that SHFL).  The store cannot move above the shared-memory atomics of the deposit.
+    if (lane == 0) s_mail[threadIdx.x >> 5] = nn;
+    __syncwarp();  // the lanes' deposits (and the mailbox) are visible below
+    nn = s_mail[threadIdx.x >> 5];
     WorkItem nnwi = nwi;
     if (nn < nitems) nnwi = bv.items[nn];
 
@@ -726,7 +743,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   __shared__ uint32_t s_next[2];
   // 128-byte aligned TMA destinations; the offset is applied to the shared-space pointer so that the loads
   // below stay LDS (a round trip through uintptr_t made them generic LD with 64-bit address arithmetic)
-  float* s_base = reinterpret_cast<float*>(s_raw + ((128u - (smem_u32(s_raw) & 127u)) & 127u));
+  float* s_base = reinterpret_cast<float*>(s_raw + ((1024u - (smem_u32(s_raw) & 1023u)) & 1023u));
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
@@ -781,8 +798,9 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   if (nxt < nitems) nwi = bv.items[nxt];
 
   while (it < nitems) {
+    uint32_t fetched = 0;  // item i+2: issued now, stored right before the barrier at the end of the item
     if (tid == 0) {
-      s_next[par] = sched_next(bv.sched);  // item i+2
+      fetched = sched_next(bv.sched);
       if (STAGES == 2 && nxt < nitems) issue(nwi, stage ^ 1);
     }
     const TileOrigin o = tile_origin(wi);
@@ -808,7 +826,9 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         const int gz = cz + zoff;
         const float4 v = make_float4(__ldg(p + wrap_hi(gz, m)), __ldg(p + wrap_hi(gz + 1, m)),
                                      __ldg(p + wrap_hi(gz + 2, m)), __ldg(p + wrap_hi(gz + 3, m)));
-        reinterpret_cast<float4*>(s_w + comp * G::COMP)[rr] = v;
+        // main plane: 16-byte chunk g of row r sits at chunk g ^ (r & 7) (the layout TMA's 128-byte swizzle writes)
+        const int rs = rr < G::NGM ? ((rr & ~7) | ((rr ^ (rr >> 3)) & 7)) : rr;
+        reinterpret_cast<float4*>(s_w + comp * G::COMP)[rs] = v;
       }
       fence_proxy_async();  // generic-proxy writes before the async proxy refills this buffer
       __syncthreads();
@@ -829,9 +849,27 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         T::template axis<GRAD>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
         T::template axis<GRAD>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
         T::template axis<GRAD>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
-        NodeCol nc[P];
+        // Byte offset of node (row, column s) in a staged component block.  MAIN plane rows are 128 bytes and
+        // carry TMA's 128-byte swizzle: 16-byte chunk g of row r sits at chunk g ^ (r & 7), so lanes at the same z
+        // in different (x, y) rows hit different banks (unswizzled, bank = z alone: ncu showed 40 % of the
+        // gather's shared wavefronts were conflict replays, LSU data pipe 87 % busy).  HALO plane: plain.
+        //   offset = row * pitch[c] + (col[c] ^ (swz(row) & mask[c]))
+        int colB[P], maskB[P], pitchB[P];
 #pragma unroll
-        for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
+        for (int c = 0; c < P; ++c) {
+          const int s = sz + (G::ZLO - G::HLO) + c;
+          const bool main = s < TZ;
+          colB[c] = main ? 4 * s : 4 * (G::MAIN + s - TZ);
+          maskB[c] = main ? 0x70 : 0;
+          pitchB[c] = main ? 4 * TZ : 4 * G::HZ;
+        }
+        const int row0 = sx * G::SY + sy;
+        const char* s_valB = reinterpret_cast<const char*>(s_val);
+        auto node_ptr = [&](int a, int b, int c) -> const float* {
+          const int row = row0 + a * G::SY + b;
+          const int swz = (row & 7) << 4;
+          return reinterpret_cast<const float*>(s_valB + (row * pitchB[c] + (colB[c] ^ (swz & maskB[c]))));
+        };
         if (!GRAD) {
           float acc[NCOMP];
 #pragma unroll
@@ -844,7 +882,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
               for (int c = 0; c < P; ++c) {
                 const float wxyz = wxy * wz[c];
-                const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
+                const float* node = node_ptr(a, b, c);
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, node[q * G::COMP], acc[q]);
               }
@@ -867,7 +905,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
               const float wdx = dx[a] * wy[b], wdy = wx[a] * dy[b], wxy = wx[a] * wy[b];
 #pragma unroll
               for (int c = 0; c < P; ++c) {
-                const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
+                const float* node = node_ptr(a, b, c);
                 float val = 0.0f;
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], node[q * G::COMP], val);
@@ -884,6 +922,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
       }
       if (last) break;
     }
+    if (tid == 0) s_next[par] = fetched;
     __syncthreads();  // every thread is done with this stage: it may be refilled
     const uint32_t nn = s_next[par];
     par ^= 1;
@@ -974,7 +1013,7 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const fl
   using G = Geo<T>;
   constexpr size_t stage_bytes = sizeof(float) * (size_t)NCOMP * G::COMP;
   constexpr int STAGES = 2 * stage_bytes <= 100 * 1024 ? 2 : 1;
-  constexpr size_t smem = STAGES * stage_bytes + 128;
+  constexpr size_t smem = STAGES * stage_bytes + 1024;  // + alignment slack of the swizzle atom
   auto kern = k_gather<T, NCOMP, GRAD, STAGES>;
   static int occ = 0;
   if (!occ) {
@@ -987,8 +1026,8 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const fl
   const int m = c->mg;
   for (int a = 0; a < NCOMP; ++a) {
     mp.p[a] = mesh[a];
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, &maps.m[2 * a]));
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::HZ, &maps.m[2 * a + 1]));
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, true, &maps.m[2 * a]));
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::HZ, false, &maps.m[2 * a + 1]));
   }
   const float a_eff = GRAD ? (float)((double)alpha * (double)c->mg / c->p.box) : alpha;
   const int3 nr = make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m));

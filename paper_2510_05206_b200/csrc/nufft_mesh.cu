@@ -42,7 +42,7 @@ int es_scatter_w<ES_W>(Ctx* c, int ncomp, const float* wsrc, int wstride, float*
 #else
 template <class T, int NCOMP, bool GRAD>
 static int go(Ctx* c, const GatherArgs& a, cudaStream_t st) {
-  constexpr size_t smem = sizeof(float) * (size_t)NCOMP * Geo<T>::COMP + 1024;
+  constexpr size_t smem = sizeof(float) * (size_t)NCOMP * Geo<T>::COMP + 128;
   if (smem > 200 * 1024) return fail(c, PM_EINVAL, "ES gather: %d meshes of width %d do not fit in shared memory", NCOMP, T::P);
   const int roll[3] = {0, 0, 0};
   return run_gather<T, NCOMP, GRAD>(c, es_params<T>(c), roll, a.mesh, a.cot, a.cstride, a.ncot, a.const_coef, a.wmul,

@@ -155,25 +155,42 @@ struct Buckets {
   uint32_t* ov_tile;   // their tiles
 };
 
+// Overflow list space is reserved per WARP in chunks of OV_CHUNK entries (one atomic on the list counter per
+// chunk, not per warp call: with half of the particles overflowing, config 4, two million same-address atomics
+// were a millisecond of their own).  ov_pos / ov_left are warp-uniform.  Entries a warp reserves and does not
+// use are holes: tile = NO_TILE, skipped by k_ov_permute.
+constexpr uint32_t OV_CHUNK = 1024;
+
+__device__ __forceinline__ void ov_fill_holes(const Buckets& bk, uint32_t ov_pos, uint32_t ov_left) {
+  for (uint32_t j = threadIdx.x & 31u; j < ov_left; j += 32) bk.ov_tile[ov_pos + j] = NO_TILE;
+}
+
 template <int MODE>
 __device__ __forceinline__ void put_record(uint4* __restrict__ rec, const Buckets& bk, uint32_t tile, uint32_t toff,
-                                           uint32_t slot, bool valid, uint4 r) {
+                                           uint32_t slot, bool valid, uint4 r, uint32_t& ov_pos, uint32_t& ov_left) {
   if (MODE == 1) {
     if (valid) rec[toff + slot] = r;
   } else if (MODE == 2) {
     const bool ov = valid && slot >= bk.capt;
     if (valid && !ov) rec[toff + slot] = r;
     const unsigned ovm = __ballot_sync(0xffffffffu, ov);
-    if (ovm) {  // one atomic per warp for its overflowing lanes
+    if (ovm) {
       const unsigned lane = threadIdx.x & 31u;
-      uint32_t base = 0;
-      if (lane == (unsigned)(__ffs(ovm) - 1)) base = atomicAdd(bk.ov_count, (uint32_t)__popc(ovm));
-      base = __shfl_sync(0xffffffffu, base, __ffs(ovm) - 1);
+      const uint32_t cnt = (uint32_t)__popc(ovm);
+      if (cnt > ov_left) {  // warp-uniform: drop the rest of the chunk, reserve a new one
+        ov_fill_holes(bk, ov_pos, ov_left);
+        uint32_t base = 0;
+        if (lane == 0) base = atomicAdd(bk.ov_count, OV_CHUNK);
+        ov_pos = __shfl_sync(0xffffffffu, base, 0);
+        ov_left = OV_CHUNK;
+      }
       if (ov) {
-        const uint32_t j = base + (uint32_t)__popc(ovm & ((1u << lane) - 1u));
+        const uint32_t j = ov_pos + (uint32_t)__popc(ovm & ((1u << lane) - 1u));
         bk.ov_rec[j] = r;
         bk.ov_tile[j] = tile;
       }
+      ov_pos += cnt;
+      ov_left -= cnt;
     }
   }
 }
@@ -193,6 +210,7 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
   const int64_t nwarps = (int64_t)gridDim.x * (BIN_BLOCK / 32);
   const float4* p4 = reinterpret_cast<const float4*>(pos);
   float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
+  uint32_t ov_pos = 0, ov_left = 0;  // this warp's reserved piece of the overflow list (MODE 2)
   if (gwarp < nchunk) {
     const float4* src = p4 + gwarp * (BIN_WARP_PART * 3 / 4);
     a = __ldcs(src + lane), b = __ldcs(src + 32 + lane), c = __ldcs(src + 64 + lane);
@@ -227,7 +245,8 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
 #pragma unroll
       for (int k = 0; k < 4; ++k)
         put_record<MODE>(rec, bk, tile[k], toff[k], slot[k], true,
-                         make_uint4(fx[k], fy[k], fz[k], (uint32_t)(ch * BIN_WARP_PART + 32 * k + (int)lane)));
+                         make_uint4(fx[k], fy[k], fz[k], (uint32_t)(ch * BIN_WARP_PART + 32 * k + (int)lane)), ov_pos,
+                         ov_left);
     }
     __syncwarp();
   }
@@ -248,22 +267,30 @@ __global__ void __launch_bounds__(BIN_BLOCK) k_bin_pass(const float* __restrict_
     if (PERMUTE) {
       uint32_t toff = 0;
       if (valid) toff = MODE == 1 ? tile_off[tile[0]] : tile[0] * bk.capt;
-      put_record<MODE>(rec, bk, tile[0], toff, slot[0], valid, make_uint4(fx, fy, fz, (uint32_t)i));
+      put_record<MODE>(rec, bk, tile[0], toff, slot[0], valid, make_uint4(fx, fy, fz, (uint32_t)i), ov_pos, ov_left);
     }
   }
+  if (MODE == 2) ov_fill_holes(bk, ov_pos, ov_left);
 }
 
-// Overflow of the single-pass path: sort the overflow list by tile into rec[ov_base + ov_off[tile] ...).
+// Overflow of the single-pass path: sort the overflow list by tile into rec[ov_base + ov_off[tile] ...).  The
+// list was appended warp by warp, so consecutive entries mostly share a tile: one atomic per run of equal tiles
+// (claim_slots), not per entry -- the dense tiles of a clustered input would otherwise serialise on a handful of
+// cursor addresses.  Holes (NO_TILE) take no slot.
 __global__ void __launch_bounds__(256) k_ov_permute(const uint32_t* __restrict__ ov_count,
                                                     const uint4* __restrict__ ov_rec,
                                                     const uint32_t* __restrict__ ov_tile,
                                                     const uint32_t* __restrict__ ov_off, uint32_t* __restrict__ ov_cur,
                                                     uint4* __restrict__ rec, uint32_t ov_base) {
   const uint32_t n = *ov_count;
-  for (uint32_t j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
-    const uint32_t t = ov_tile[j];
-    const uint32_t slot = atomicAdd(&ov_cur[t], 1u);
-    rec[ov_base + ov_off[t] + slot] = ov_rec[j];
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t stride = gridDim.x * blockDim.x;
+  for (uint32_t b = blockIdx.x * blockDim.x + (threadIdx.x & ~31u); b < n; b += stride) {  // warp-uniform
+    const uint32_t j = b + lane;
+    uint32_t key[1] = {NO_TILE}, slot[1] = {0};
+    if (j < n) key[0] = ov_tile[j];
+    claim_slots<true, 1>(ov_cur, key, slot);
+    if (key[0] != NO_TILE) rec[ov_base + ov_off[key[0]] + slot[0]] = ov_rec[j];
   }
 }
 

@@ -259,8 +259,11 @@ static int build(Ctx* c) {
   PM_CUDA(c, cudaMalloc((void**)&c->rec, sizeof(uint4) * ((size_t)c->ov_base + (size_t)c->cap)));
   if (c->bin_capt) {
     PM_CUDA(c, cudaMalloc((void**)&c->ov_count, sizeof(uint32_t)));
-    PM_CUDA(c, cudaMalloc((void**)&c->ov_rec, sizeof(uint4) * (size_t)(c->cap > 0 ? c->cap : 1)));
-    PM_CUDA(c, cudaMalloc((void**)&c->ov_tile, sizeof(uint32_t) * (size_t)(c->cap > 0 ? c->cap : 1)));
+    // + reserved-but-unused list space (holes): < 32 of every 1024-entry chunk, and one open chunk per resident
+    // binning warp at the end of the pass
+    const size_t ov_len = (size_t)c->cap + (size_t)c->cap / 16 + ((size_t)c->num_sms * c->bin_occ * 8 + 1) * 1024;
+    PM_CUDA(c, cudaMalloc((void**)&c->ov_rec, sizeof(uint4) * ov_len));
+    PM_CUDA(c, cudaMalloc((void**)&c->ov_tile, sizeof(uint32_t) * ov_len));
     PM_CUDA(c, cudaMalloc((void**)&c->ov_cur, sizeof(uint32_t) * (size_t)c->ntiles));
   }
   PM_CUDA(c, cudaMalloc((void**)&c->tile_cnt, sizeof(uint32_t) * (size_t)c->ntiles));

@@ -126,7 +126,7 @@ struct Geo {
   static constexpr int HZ = ZLO + (HHI + 3) / 4 * 4;                 // halo columns per row
   static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, NROW = SX * SY;
   static constexpr int MAIN = NROW * TZ, HAL = NROW * HZ;            // words per component
-  static constexpr int COMP = (MAIN + HAL + 255) / 256 * 256;        // component block (1024-byte multiple: TMA swizzle atom)
+  static constexpr int COMP = (MAIN + HAL + 31) / 32 * 32;           // component block (128-byte multiple)
   static constexpr int NGM = NROW * (TZ / 4), NGH = NROW * (HZ / 4); // float4 groups per component
   static constexpr int NGROUP = NGM + NGH;
   static_assert(TZ == 32, "the main plane's row pitch must be 32 words");
@@ -743,7 +743,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   __shared__ uint32_t s_next[2];
   // 128-byte aligned TMA destinations; the offset is applied to the shared-space pointer so that the loads
   // below stay LDS (a round trip through uintptr_t made them generic LD with 64-bit address arithmetic)
-  float* s_base = reinterpret_cast<float*>(s_raw + ((1024u - (smem_u32(s_raw) & 1023u)) & 1023u));
+  float* s_base = reinterpret_cast<float*>(s_raw + ((128u - (smem_u32(s_raw) & 127u)) & 127u));
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
@@ -826,9 +826,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         const int gz = cz + zoff;
         const float4 v = make_float4(__ldg(p + wrap_hi(gz, m)), __ldg(p + wrap_hi(gz + 1, m)),
                                      __ldg(p + wrap_hi(gz + 2, m)), __ldg(p + wrap_hi(gz + 3, m)));
-        // main plane: 16-byte chunk g of row r sits at chunk g ^ (r & 7) (the layout TMA's 128-byte swizzle writes)
-        const int rs = rr < G::NGM ? ((rr & ~7) | ((rr ^ (rr >> 3)) & 7)) : rr;
-        reinterpret_cast<float4*>(s_w + comp * G::COMP)[rs] = v;
+        reinterpret_cast<float4*>(s_w + comp * G::COMP)[rr] = v;
       }
       fence_proxy_async();  // generic-proxy writes before the async proxy refills this buffer
       __syncthreads();
@@ -849,27 +847,12 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         T::template axis<GRAD>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
         T::template axis<GRAD>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
         T::template axis<GRAD>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
-        // Byte offset of node (row, column s) in a staged component block.  MAIN plane rows are 128 bytes and
-        // carry TMA's 128-byte swizzle: 16-byte chunk g of row r sits at chunk g ^ (r & 7), so lanes at the same z
-        // in different (x, y) rows hit different banks (unswizzled, bank = z alone: ncu showed 40 % of the
-        // gather's shared wavefronts were conflict replays, LSU data pipe 87 % busy).  HALO plane: plain.
-        //   offset = row * pitch[c] + (col[c] ^ (swz(row) & mask[c]))
-        int colB[P], maskB[P], pitchB[P];
+        // (TMA's 128-byte swizzle of the MAIN plane was measured: it is correct but RAISES the bank conflicts of
+        // Lagrangian-ordered particles from 85 M to 136 M wavefronts, 1.09 -> 1.21 ms: with a row pitch of 32 words
+        // lanes at distinct z already sit in distinct banks, and the swizzle scatters them.)
+        NodeCol nc[P];
 #pragma unroll
-        for (int c = 0; c < P; ++c) {
-          const int s = sz + (G::ZLO - G::HLO) + c;
-          const bool main = s < TZ;
-          colB[c] = main ? 4 * s : 4 * (G::MAIN + s - TZ);
-          maskB[c] = main ? 0x70 : 0;
-          pitchB[c] = main ? 4 * TZ : 4 * G::HZ;
-        }
-        const int row0 = sx * G::SY + sy;
-        const char* s_valB = reinterpret_cast<const char*>(s_val);
-        auto node_ptr = [&](int a, int b, int c) -> const float* {
-          const int row = row0 + a * G::SY + b;
-          const int swz = (row & 7) << 4;
-          return reinterpret_cast<const float*>(s_valB + (row * pitchB[c] + (colB[c] ^ (swz & maskB[c]))));
-        };
+        for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
         if (!GRAD) {
           float acc[NCOMP];
 #pragma unroll
@@ -882,7 +865,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
               for (int c = 0; c < P; ++c) {
                 const float wxyz = wxy * wz[c];
-                const float* node = node_ptr(a, b, c);
+                const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, node[q * G::COMP], acc[q]);
               }
@@ -905,7 +888,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
               const float wdx = dx[a] * wy[b], wdy = wx[a] * dy[b], wxy = wx[a] * wy[b];
 #pragma unroll
               for (int c = 0; c < P; ++c) {
-                const float* node = node_ptr(a, b, c);
+                const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
                 float val = 0.0f;
 #pragma unroll
                 for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], node[q * G::COMP], val);
@@ -1013,7 +996,7 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const fl
   using G = Geo<T>;
   constexpr size_t stage_bytes = sizeof(float) * (size_t)NCOMP * G::COMP;
   constexpr int STAGES = 2 * stage_bytes <= 100 * 1024 ? 2 : 1;
-  constexpr size_t smem = STAGES * stage_bytes + 1024;  // + alignment slack of the swizzle atom
+  constexpr size_t smem = STAGES * stage_bytes + 128;
   auto kern = k_gather<T, NCOMP, GRAD, STAGES>;
   static int occ = 0;
   if (!occ) {
@@ -1026,7 +1009,7 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const fl
   const int m = c->mg;
   for (int a = 0; a < NCOMP; ++a) {
     mp.p[a] = mesh[a];
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, true, &maps.m[2 * a]));
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, false, &maps.m[2 * a]));
     PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::HZ, false, &maps.m[2 * a + 1]));
   }
   const float a_eff = GRAD ? (float)((double)alpha * (double)c->mg / c->p.box) : alpha;

@@ -54,7 +54,10 @@ typedef struct pm_params {
   double coeff;        /* C in Lap(phi) = C * delta, g = -grad(phi) (Eq. 2.1-2.2, R11)      */
   double nufft_sigma;  /* upsampling factor sigma (5/4; BASELINE config 3: 2)                */
   double nufft_eps;    /* requested NUFFT tolerance                                         */
-  int64_t max_particles; /* capacity of the binning workspace; N of every call must be <= this             */
+  int64_t max_particles; /* capacity of the binning workspace; N of every call must be <= this.  The ctx       */
+                         /* allocates about 68 bytes per particle for it (tile buckets of twice the mean load,  */
+                         /* overflow segment and list: DESIGN.md section 6); PMF_BIN_TWOPASS=1 in the           */
+                         /* environment at pm_create selects the 16 bytes per particle two-pass sort instead    */
 } pm_params;
 
 /* ---- lifetime ------------------------------------------------------------------------------------- */

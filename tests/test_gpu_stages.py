@@ -244,6 +244,28 @@ def test_bucket_overflow_of_single_pass_binning(pm):
         pm.pm_destroy(ctx)
 
 
+def test_two_pass_binning_path_matches(pm, monkeypatch):
+    """The two-pass (histogram + permute) binning, kept for N too large for 32-bit bucket indices and selectable
+    with PMF_BIN_TWOPASS=1, must give the same assignment and forces as the default single-pass path."""
+    pos, c = gen.make_config_positions("cfg4", n_p=32)
+    n = pos.shape[0]
+    f = gen.random_mesh(c["m"], 6, 3)
+    ref = po.scatter(pos, c["m"], c["box"], 2)
+    outs = []
+    for two_pass in ("0", "1"):
+        monkeypatch.setenv("PMF_BIN_TWOPASS", two_pass)
+        ctx = pm.pm_create(pm.PMParams(m=c["m"], box=c["box"], max_particles=n, worder=2))
+        mesh = torch.zeros(c["m"], c["m"], c["m"], device="cuda")
+        pm.pm_assign(ctx, dev(pos), None, mesh)
+        out = torch.empty(n, 3, device="cuda")
+        pm.pm_interp(ctx, [dev(f[a]) for a in range(3)], dev(pos), out)
+        assert rel_l2(mesh.cpu().numpy(), ref) <= 1e-6
+        outs.append(out.cpu().numpy())
+        pm.pm_destroy(ctx)
+    # the gather of one particle does not depend on how the records were sorted
+    assert np.array_equal(outs[0], outs[1])
+
+
 def test_errors_are_reported(pm):
     with pytest.raises(pm.PMError):
         pm.pm_create(pm.PMParams(m=30, box=1.0, max_particles=10))  # m not a multiple of 4

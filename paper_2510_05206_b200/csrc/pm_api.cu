@@ -39,11 +39,14 @@ int assign_ctx_meshes(Ctx* c, const ShiftSplit& sh, bool second_grid, cudaStream
   if (!c->zero_done) PM_CUDA(c, cudaMemsetAsync(c->rho[0], 0, sizeof(float) * (size_t)c->G, st));
   c->zero_done = false;  // consumed: a second evaluation in the same call clears the mesh itself
   if (c->p.method == 0) {
-    PM_TRY(launch_scatter(c, c->p.worder, sh, 1, nullptr, 0, &c->rho[0], st));
-    if (second_grid) {
-      PM_CUDA(c, cudaMemsetAsync(c->rho[1], 0, sizeof(float) * (size_t)c->G, st));
-      PM_TRY(launch_scatter(c, c->p.worder, half_cell(c), 1, nullptr, 0, &c->rho[1], st));
+    c->scatter_mesh_zeroed = true;  // the ctx meshes were just cleared: exclusive tile interiors may be stored
+    int rc = launch_scatter(c, c->p.worder, sh, 1, nullptr, 0, &c->rho[0], st);
+    if (rc == PM_OK && second_grid) {
+      rc = (cudaMemsetAsync(c->rho[1], 0, sizeof(float) * (size_t)c->G, st) == cudaSuccess) ? PM_OK : PM_ECUDA;
+      if (rc == PM_OK) rc = launch_scatter(c, c->p.worder, half_cell(c), 1, nullptr, 0, &c->rho[1], st);
     }
+    c->scatter_mesh_zeroed = false;
+    PM_TRY(rc);
   } else {
     PM_TRY(launch_es_scatter(c, 1, nullptr, 0, &c->rho[0], st));
   }

@@ -414,7 +414,7 @@ __global__ void __launch_bounds__(256) k_items(const uint32_t* __restrict__ tile
   const uint32_t per = k ? (e - b + k - 1) / k : 0;  // even split: no tiny remainder items
   for (uint32_t j = 0; j < k; ++j) {  // exactly the k slots the scan reserved (a slot may stay empty)
     WorkItem w;
-    w.tile = (uint32_t)t;
+    w.tile = (uint32_t)t | (k == 1 ? 0x80000000u : 0u);  // single item: exclusive interior (see k_scatter_warp)
     w.begin = min(b + j * per, e);
     w.end = min(w.begin + per, e);
     w.txyz = txyz;
@@ -447,7 +447,7 @@ __global__ void __launch_bounds__(256) k_items_bucketed(const uint32_t* __restri
     const uint32_t per = k ? (e - b + k - 1) / k : 0;
     for (uint32_t j = 0; j < k; ++j) {
       WorkItem w;
-      w.tile = (uint32_t)t;
+      w.tile = (uint32_t)t | ((k == 1 && ov == 0) ? 0x80000000u : 0u);  // the tile's only item
       w.begin = min(b + j * per, e);
       w.end = min(w.begin + per, e);
       w.txyz = txyz;

@@ -35,7 +35,7 @@ constexpr uint32_t REC_ONE = 1u << REC_FRAC;
 constexpr uint32_t REC_MASK = REC_ONE - 1u;
 
 struct WorkItem {
-  uint32_t tile, begin, end;
+  uint32_t tile, begin, end;  // tile: bit 31 set = this item holds ALL particles of its tile (exclusive interior)
   uint32_t txyz;  // tile coordinates packed tx | ty << 10 | tz << 20 (written by k_items: no division in the hot kernels)
 };
 
@@ -99,6 +99,7 @@ struct Ctx {
   void* zero_req;
   size_t zero_req_bytes;
   bool zero_done;  // rho[0] was cleared by the binning pass of this call
+  bool scatter_mesh_zeroed;  // hint for the next scatter launch: its target mesh is all zero (pm_force's own meshes)
   int nufft_w;
   double nufft_beta;
 

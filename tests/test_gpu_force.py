@@ -100,6 +100,28 @@ def test_force_parity_kernels_and_interlacing(pm, worder, interlace):
     assert err <= FORCE_TOL, err
 
 
+@pytest.mark.parametrize("m", [24, 40, 72])
+@pytest.mark.parametrize("interlace", [0, 1])
+def test_force_parity_ragged_tiles(pm, m, interlace):
+    """Meshes that are not a multiple of the 8 x 8 x 32 tile (a ragged last tile per axis, m = 24: a single
+    tile shorter than TZ whose halo wraps onto itself) and half of the particles inside one tile (a tile split
+    over several work items beside single-item tiles): exercises the stored (exclusive) and the reduced
+    parts of the CIC scatter flush of pm_force, with and without the shifted second grid."""
+    rng = np.random.default_rng(100 + m)
+    n = 40000
+    box = float(m)
+    pu = rng.random((n // 2, 3)) * box
+    pc = rng.random((n - n // 2, 3)) * np.array([7.5, 7.5, min(m, 31.5)]) + np.array([8.0, 8.0, 0.0])
+    pos = np.concatenate([pu, pc]).astype(np.float32) % np.float32(box)
+    pos = pos[rng.permutation(n)]
+    c = dict(m=m, box=box, worder=2, interlace=interlace, grad_order=4, lap_order=0, deconv_pow=2)
+    f = gpu_force(pm, params_of(pm, c, n), pos)
+    ref = po.force(pos, m, box, **oracle_kw(c))
+    err = rel_l2(f, ref)
+    record_error(f"force/ragged-m={m}/interlace={interlace}", err, FORCE_TOL)
+    assert err <= FORCE_TOL, err
+
+
 def test_zero_force_on_lattice(pm):
     """Uniform lattice => zero force (R7), m = n_p and m = 2 n_p."""
     for m in (32, 64):

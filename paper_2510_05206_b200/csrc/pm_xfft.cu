@@ -24,7 +24,13 @@
 namespace pmf {
 
 constexpr int XC = 8;    // (y,z) columns per CTA: 64 contiguous bytes of every x plane
-constexpr int XEPT = 16; // elements per thread -> N * XC / 16 threads per CTA
+#ifndef PMF_XEPT
+#define PMF_XEPT 16  // 8 (512 threads, 2 CTAs/SM at m = 512) was measured: 0.85 ms instead of 0.83 ms
+#endif
+#ifndef PMF_XTW_DERIVE
+#define PMF_XTW_DERIVE 1
+#endif
+constexpr int XEPT = PMF_XEPT; // elements per thread -> N * XC / XEPT threads per CTA
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
@@ -141,16 +147,37 @@ __device__ __forceinline__ void xfft_stage(const float2* __restrict__ tw, int ti
     float2 v[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) v[r] = ld(p0 + r * M, c);
-    if (INV) {
-      if (M > 1)  // M = 1: j = 0, every twiddle is 1
+    // twiddles W^{j r}, r = 1 .. R-1: the powers of two are loaded, the others are products of two of them (one
+    // rounding more, ~1e-7): 3 instead of 7 table loads per radix-8 butterfly -- the kernel is bound by the
+    // load/store pipe (ncu: 64 % busy, a third of its instructions in these stages were twiddle loads).
+    float2 w[R];
+    if (M > 1) {  // M = 1: j = 0, every twiddle is 1
 #pragma unroll
-        for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], __ldg(tw + (N / S) * j * r));
+      for (int r = 1; r < R; r <<= 1) w[r] = __ldg(tw + (N / S) * j * r);
+#if PMF_XTW_DERIVE
+#pragma unroll
+      for (int r = 3; r < R; ++r)
+        if (r & (r - 1)) {  // not a power of two: highest set bit times the rest
+          int hb = 1;
+          while (hb * 2 <= r) hb *= 2;
+          w[r] = cmulx(w[hb], w[r - hb]);
+        }
+#else
+#pragma unroll
+      for (int r = 3; r < R; ++r)
+        if (r & (r - 1)) w[r] = __ldg(tw + (N / S) * j * r);
+#endif
+    }
+    if (INV) {
+      if (M > 1)
+#pragma unroll
+        for (int r = 1; r < R; ++r) v[r] = cmulc(v[r], w[r]);
       Dft<R, 1>::run(v);
     } else {
       Dft<R, -1>::run(v);
       if (M > 1)
 #pragma unroll
-        for (int q = 1; q < R; ++q) v[q] = cmulx(v[q], __ldg(tw + (N / S) * j * q));
+        for (int q = 1; q < R; ++q) v[q] = cmulx(v[q], w[q]);
     }
 #pragma unroll
     for (int q = 0; q < R; ++q) st(p0 + q * M, c, v[q]);
@@ -211,7 +238,7 @@ struct XTabs {
 //   MODE 1 (transpose): in0..2 -> out0 (, out1) = x-inverse of sum_a conj(S_a) ghat_a
 // Every input is the (y,z)-transformed, x-untransformed spectrum [x][y][hz]; every output likewise.
 template <int N, int MODE>
-__global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? 3 : 1) k_xfft_kspace(XTabs t, const float2* __restrict__ in0,
+__global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? (XEPT >= 16 ? 3 : 2) : 1) k_xfft_kspace(XTabs t, const float2* __restrict__ in0,
                                                                const float2* __restrict__ in1,
                                                                const float2* __restrict__ in2,
                                                                float2* __restrict__ out0, float2* __restrict__ out1,

@@ -246,7 +246,9 @@ __device__ __forceinline__ void load_rec(uint4& r, const BinView& bv, uint32_t i
 // resident CTAs per SM the register allocation aims at (the unit-weight CIC assign is the headline kernel)
 template <class T, int NCOMP, bool WEIGHTED>
 constexpr int scatter_min_ctas() {
-  return (NCOMP == 1 && !WEIGHTED) ? (T::P == 2 ? 4 : (T::P <= 4 ? 3 : 1)) : (NCOMP == 1 ? 2 : 1);
+  // vector scatter of the VJP (3 components): at 151 registers ONE CTA was resident per SM (ncu: 12.5 % warps
+  // active, 3.5 ms at 512^3); two CTAs for CIC / TSC cap the allocation at 128
+  return (NCOMP == 1 && !WEIGHTED) ? (T::P == 2 ? 4 : (T::P <= 4 ? 3 : 1)) : (NCOMP == 1 ? 2 : (T::P <= 3 ? 2 : 1));
 }
 template <class T, int NCOMP, bool WEIGHTED, int NBUF>
 __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>()) k_scatter(BinView bv, typename T::Params tp, int3 roll,

@@ -49,16 +49,29 @@ typedef struct pm_params {
   int32_t grad_order;  /* 0 exact i k; 2, 4, 6 finite-difference symbol (Table 2)        */
   int32_t lap_order;   /* 0 exact -k^2; 2, 4, 6 finite-difference symbol (Table 2)                        */
   int32_t method;      /* 0 PM (Sec. 2.5); 1 NUFFT                     */
-  int32_t nufft_width; /* ES-kernel width w in fine cells, 2..16; 0 = from nufft_eps (R10)                */
+  int32_t nufft_width; /* ES-kernel width w in fine cells, 4..8 (the widths built); 0 = from nufft_eps (R10)  */
   double box;          /* box size L > 0                                                                   */
   double coeff;        /* C in Lap(phi) = C * delta, g = -grad(phi) (Eq. 2.1-2.2, R11)      */
   double nufft_sigma;  /* upsampling factor sigma (5/4; BASELINE config 3: 2)                */
   double nufft_eps;    /* requested NUFFT tolerance                                         */
   int64_t max_particles; /* capacity of the binning workspace; N of every call must be <= this.  The ctx       */
                          /* allocates about 68 bytes per particle for it (tile buckets of twice the mean load,  */
-                         /* overflow segment and list: DESIGN.md section 6); PMF_BIN_TWOPASS=1 in the           */
-                         /* environment at pm_create selects the 16 bytes per particle two-pass sort instead    */
+                         /* overflow segment and list: DESIGN.md section 6); PM_FLAG_BIN_TWOPASS selects the    */
+                         /* 16 bytes per particle two-pass sort instead                                         */
+  int32_t flags;         /* PM_FLAG_* bits, 0 = defaults                                                        */
+  int32_t reserved;      /* must be 0                                                                           */
 } pm_params;
+
+/* pm_params.flags.  No environment variable steers the library. */
+#define PM_FLAG_BIN_TWOPASS 1 /* a0: histogram + permute counting sort (two reads of the positions, 16 B/particle of
+                                 workspace) instead of the single-pass bucketed sort */
+#define PM_FLAG_NO_XFUSE 2    /* a2-a4: 3-D cuFFT + pointwise Fourier-space kernel instead of the fused x-FFT kernel */
+#define PM_FLAG_GRAD_REAL 4   /* a3-a4, method 0, grad_order 2/4/6: apply the gradient as the real-space stencil of
+                                 Table 2 ("Real" column; its DFT IS the Fourier symbol) to the
+                                 potential mesh: ONE inverse FFT instead of three.  Same operator, other rounding. */
+#define PM_FLAG_KERNEL_GRAD 8 /* method 1: force from the gradient of the ES kernel ("SPH-like"):
+                                 the potential is interpolated with grad(phi_ES) instead of multiplying by i k.
+                                 pm_force only (its VJP would need second derivatives of the kernel: PM_ESTATE). */
 
 /* ---- lifetime ------------------------------------------------------------------------------------- */
 /* Validates p, builds cuFFT plans, symbol tables and workspace on the current CUDA device.  *out is set

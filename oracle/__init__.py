@@ -11,5 +11,10 @@ Modules
                   Poisson + gradient + deconvolution (Sec. 2.5, Table 2), interlacing,
                   full force and its reverse-mode VJP (App. C rule table).
   nufft_oracle -- brute-force non-uniform DFT force (Eq. 2.18-2.19) and the
-                  exponential-of-semicircle NUFFT stage by stage (Sec. 2.5).
+                  exponential-of-semicircle NUFFT stage by stage (Sec. 2.5), with the
+                  i k gradient or the gradient of the kernel (:264).
+  dkd_oracle   -- drift-kick-drift step (Eq. 2.14) and the backward-in-time adjoint
+                  step, Table 3 row by row.
+  analysis_oracle -- binned (cross-)power spectrum of the interlaced, deconvolved
+                  density (:375); sheet-based resampling, trilinear variant (:369-371).
 """

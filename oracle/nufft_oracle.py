@@ -183,6 +183,26 @@ def nufft_kspace(fine, m: int, box: float, n_particles: int, w: int, beta: float
     return [np.fft.irfftn(Ma * F, s=(m_fine,) * 3, axes=(0, 1, 2)) * float(m_fine) ** 3 for Ma in M]
 
 
+def nufft_kspace_potential(fine, m: int, box: float, n_particles: int, w: int, beta: float, coeff: float = 1.0):
+    """Spread grid -> fine POTENTIAL grid phi, ready for interpolation with the ES kernel or its gradient:
+    phi_hat = coeff * delta_hat / (-k^2) (Eq. 2.2 :84) on the retained modes, divided by phi_ES_hat twice
+    (:262).  The force of the 'kernel gradient' option (:264) is -grad of its interpolant."""
+    fine = np.asarray(fine, dtype=np.float64)
+    m_fine = fine.shape[0]
+    h = m_fine // 2 + 1
+    nf = np.fft.fftfreq(m_fine, 1.0 / m_fine)
+    keep = np.abs(nf) < 0.5 * m
+    ph1 = es_kernel_ft(nf, m_fine, w, beta)
+    k1 = (2.0 * np.pi / box) * nf
+    k2 = (k1 * k1)[:, None, None] + (k1 * k1)[None, :, None] + (k1 * k1)[None, None, :h]
+    k2[0, 0, 0] = 1.0
+    mask = keep[:, None, None] & keep[None, :, None] & keep[None, None, :h]
+    phat = ph1[:, None, None] * ph1[None, :, None] * ph1[None, None, :h]
+    P = np.where(mask, -(coeff / n_particles) / (k2 * phat * phat), 0.0)
+    P[0, 0, 0] = 0.0
+    return np.fft.irfftn(P * np.fft.rfftn(fine), s=(m_fine,) * 3, axes=(0, 1, 2)) * float(m_fine) ** 3
+
+
 def nufft_kspace_vjp(fine_cot, m: int, box: float, n_particles: int, w: int, beta: float, coeff: float = 1.0):
     """Transpose of ``nufft_kspace``: sum_a F^H conj(M_a) F fine_cot_a."""
     m_fine = np.asarray(fine_cot[0]).shape[0]
@@ -192,14 +212,19 @@ def nufft_kspace_vjp(fine_cot, m: int, box: float, n_particles: int, w: int, bet
 
 
 def nufft_force(pos, m: int, box: float, sigma: float = 2.0, eps: float = 1e-6, width: int = 0,
-                coeff: float = 1.0, beta: float | None = None):
-    """Per-particle acceleration [N, 3] through the ES-kernel NUFFT (Sec. 2.5)."""
+                coeff: float = 1.0, beta: float | None = None, kernel_grad: bool = False):
+    """Per-particle acceleration [N, 3] through the ES-kernel NUFFT (Sec. 2.5).  kernel_grad: the
+    gradient is taken of the interpolation kernel ("similarly to ... smoothed-particle hydrodynamics",
+    :264) instead of multiplying by i k: g_i = -grad_X sum_j phi_j prod_a phi_ES(2 (j_a - u_a)/w)."""
     w, b = es_params(eps, sigma, width)
     if beta is not None:
         b = beta
     m_fine = int(round(sigma * m))
     n = np.asarray(pos).shape[0]
     fine = es_spread(pos, m_fine, box, w, b)
+    if kernel_grad:
+        phi = nufft_kspace_potential(fine, m, box, n, w, b, coeff)
+        return np.stack([-es_interp(phi, pos, box, w, b, deriv_axis=a) for a in range(3)], axis=1)
     g = nufft_kspace(fine, m, box, n, w, b, coeff)
     return np.stack([es_interp(g[a], pos, box, w, b) for a in range(3)], axis=1)
 

@@ -10,7 +10,8 @@ Pins (tests/test_oracle_*.py, all ``-m "not gpu"``): brute-force Eq. C.1 / C.2 o
 with W taken from the piecewise definition; partition of unity and first moment of Table 1;
 adjointness Eq. C.14; mesh-injection closed form for every (grad, lap) order of Table 2; DFT of
 the printed stencils equals the printed symbols; zero force on a lattice; momentum
-conservation; plane-wave sheet force; central finite differences for the VJP.
+conservation; plane-wave sheet force; central finite differences for the VJP and the JVPs
+(Eq. C.13), JVP/VJP duality; the real-space stencils of Table 2 against their Fourier symbols.
 Parity unpinned (GPU-vs-oracle only): the CIC position-VJP for particles that sit exactly on
 a mesh node (R12: the derivative of W is discontinuous there).
 """
@@ -19,6 +20,25 @@ from __future__ import annotations
 import numpy as np
 
 SUPPORT = {2: 2, 3: 3, 4: 4}  # worder -> nodes per axis (Table 1 :223-229, "Discrete support")
+
+# The FFT is a library step (:244).  FFT_WORKERS = 1: numpy.fft.  FFT_WORKERS != 1: the same transforms
+# through scipy.fft (pocketfft as well) with that many host threads (-1 = all) -- set by the full-size
+# parity tests (1024^3 meshes) and by bench.py's all-cores timing; the arithmetic is unchanged.
+FFT_WORKERS = 1
+
+
+def _rfftn(a):
+    if FFT_WORKERS == 1:
+        return np.fft.rfftn(a)
+    import scipy.fft as sfft
+    return sfft.rfftn(a, workers=FFT_WORKERS)
+
+
+def _irfftn(a, m):
+    if FFT_WORKERS == 1:
+        return np.fft.irfftn(a, s=(m, m, m), axes=(0, 1, 2))
+    import scipy.fft as sfft
+    return sfft.irfftn(a, s=(m, m, m), axes=(0, 1, 2), workers=FFT_WORKERS)
 
 
 # --------------------------------------------------------------------------------------
@@ -94,17 +114,22 @@ def node_weights(u, worder: int, deriv: bool = False):
 # --------------------------------------------------------------------------------------
 # O3: scatter, Eq. C.1 (:864); adds onto the caller's mesh (:884)
 # --------------------------------------------------------------------------------------
-def scatter(pos, m: int, box: float, worder: int, weights=None, shift=None, mesh=None):
-    """rho_j += sum_i w_i W(r_j - X_i + s); returns the fp64 mesh [m, m, m]."""
+def scatter(pos, m: int, box: float, worder: int, weights=None, shift=None, mesh=None,
+            deriv_axis: int | None = None):
+    """rho_j += sum_i w_i W(r_j - X_i + s); returns the fp64 mesh [m, m, m].  With deriv_axis = a the
+    kernel is replaced by dW_j(X_i)/dX_i^a = -grad_a W(r_j - X_i) (length units; the scatter of the
+    JVP rule Eq. C.6 / C.13a)."""
     u = cell_coords(pos, m, box, shift)
     n = u.shape[0]
     w = np.ones(n) if weights is None else np.asarray(weights).astype(np.float64)
+    if deriv_axis is not None:
+        w = w * (m / box)
     if mesh is None:
         mesh = np.zeros((m, m, m), dtype=np.float64)
     p = SUPPORT[worder]
-    jx, Wx = node_weights(u[:, 0], worder)
-    jy, Wy = node_weights(u[:, 1], worder)
-    jz, Wz = node_weights(u[:, 2], worder)
+    jx, Wx = node_weights(u[:, 0], worder, deriv=(deriv_axis == 0))
+    jy, Wy = node_weights(u[:, 1], worder, deriv=(deriv_axis == 1))
+    jz, Wz = node_weights(u[:, 2], worder, deriv=(deriv_axis == 2))
     flat = mesh.reshape(-1)
     for a in range(p):
         ia = np.mod(jx + a, m)
@@ -171,6 +196,39 @@ def gather_bruteforce(mesh, pos, box, worder, shift=None):
     Wy = kernel_W(_min_image(j[None, :] - u[:, 1:2], m), worder)
     Wz = kernel_W(_min_image(j[None, :] - u[:, 2:3], m), worder)
     return np.einsum("abc,ia,ib,ic->i", mesh, Wx, Wy, Wz)
+
+
+# --------------------------------------------------------------------------------------
+# Forward-mode rules, Eq. C.13 (:943-945), rule table :956-960
+# --------------------------------------------------------------------------------------
+def scatter_jvp(pos, m: int, box: float, worder: int, weights=None, pos_tan=None, w_tan=None,
+                shift=None, mesh_tan=None):
+    """Eq. C.13a: rho~_j = rho~_in,j + sum_i [ w~_i W_j(X_i) - w_i X~_i . grad W_j(X_i) ].
+    -grad W_j(X_i) = dW_j/dX_i (:860), so the second term is a scatter with the derivative kernel of
+    each axis weighted by w_i X~_i^a.  Adds onto ``mesh_tan`` (= rho~_in, Eq. C.4)."""
+    n = np.asarray(pos).shape[0]
+    w = np.ones(n) if weights is None else np.asarray(weights).astype(np.float64)
+    out = np.zeros((m, m, m)) if mesh_tan is None else np.array(mesh_tan, dtype=np.float64)
+    if w_tan is not None:
+        scatter(pos, m, box, worder, weights=np.asarray(w_tan).astype(np.float64), shift=shift, mesh=out)
+    if pos_tan is not None:
+        t = np.asarray(pos_tan).astype(np.float64)
+        for a in range(3):
+            scatter(pos, m, box, worder, weights=w * t[:, a], shift=shift, mesh=out, deriv_axis=a)
+    return out
+
+
+def gather_jvp(mesh, pos, box: float, worder: int, pos_tan=None, mesh_tan=None, shift=None):
+    """Eq. C.13b: v~_i = sum_j [ rho~_j W_j(X_i) - rho_j X~_i . grad W_j(X_i) ]."""
+    n = np.asarray(pos).shape[0]
+    out = np.zeros(n)
+    if mesh_tan is not None:
+        out += gather(mesh_tan, pos, box, worder, shift=shift)
+    if pos_tan is not None:
+        t = np.asarray(pos_tan).astype(np.float64)
+        for a in range(3):
+            out += t[:, a] * gather(mesh, pos, box, worder, shift=shift, deriv_axis=a)
+    return out
 
 
 # --------------------------------------------------------------------------------------
@@ -278,11 +336,11 @@ def poisson_force(delta_mesh, box: float, worder: int, grad_order: int, lap_orde
     two spectra are first combined as 1/2 [d1 + e^{-ik.s} d2] (O9 mode 1, reading R1)."""
     d = np.asarray(delta_mesh, dtype=np.float64)
     m = d.shape[0]
-    dh = np.fft.rfftn(d)
+    dh = _rfftn(d)
     if delta_mesh2 is not None:
-        dh = 0.5 * (dh + interlace_phase_3d(m) * np.fft.rfftn(np.asarray(delta_mesh2, dtype=np.float64)))
+        dh = 0.5 * (dh + interlace_phase_3d(m) * _rfftn(np.asarray(delta_mesh2, dtype=np.float64)))
     S = force_symbols(m, box, worder, grad_order, lap_order, deconv_pow, coeff)
-    return [np.fft.irfftn(Sa * dh, s=(m, m, m), axes=(0, 1, 2)) for Sa in S]
+    return [_irfftn(Sa * dh, m) for Sa in S]
 
 
 def poisson_force_vjp(force_cot, box, worder, grad_order, lap_order, deconv_pow, coeff=1.0,
@@ -291,11 +349,58 @@ def poisson_force_vjp(force_cot, box, worder, grad_order, lap_order, deconv_pow,
     for the interlaced combination returns (cot of grid 1, cot of grid 2)."""
     m = np.asarray(force_cot[0]).shape[0]
     S = force_symbols(m, box, worder, grad_order, lap_order, deconv_pow, coeff)
-    q = sum(np.conj(Sa) * np.fft.rfftn(np.asarray(g, dtype=np.float64)) for Sa, g in zip(S, force_cot))
+    q = sum(np.conj(Sa) * _rfftn(np.asarray(g, dtype=np.float64)) for Sa, g in zip(S, force_cot))
     if not interlace:
-        return np.fft.irfftn(q, s=(m, m, m), axes=(0, 1, 2))
-    return (np.fft.irfftn(0.5 * q, s=(m, m, m), axes=(0, 1, 2)),
-            np.fft.irfftn(0.5 * np.conj(interlace_phase_3d(m)) * q, s=(m, m, m), axes=(0, 1, 2)))
+        return _irfftn(q, m)
+    return (_irfftn(0.5 * q, m), _irfftn(0.5 * np.conj(interlace_phase_3d(m)) * q, m))
+
+
+# --------------------------------------------------------------------------------------
+# Table 2, "Real" column (:231-242): the finite-difference gradient as a real-space stencil
+# --------------------------------------------------------------------------------------
+GRAD_STENCIL = {2: (2.0, (1.0,)), 4: (12.0, (8.0, -1.0)), 6: (60.0, (45.0, -9.0, 1.0))}
+# order -> (denominator, coefficients of offsets +1, +2, ...; antisymmetric: offset -s carries -c_s)
+# Table 2: 1/2 [-1 0 1], 1/12 [1 -8 0 8 -1], 1/60 [-1 9 -45 0 45 -9 1]
+
+
+def fd_gradient_real(phi, box: float, order: int, axis: int):
+    """d phi / d x_axis with the stencil printed in Table 2 for this order, periodic mesh."""
+    phi = np.asarray(phi, dtype=np.float64)
+    m = phi.shape[0]
+    den, coef = GRAD_STENCIL[order]
+    out = np.zeros_like(phi)
+    for s_, c in enumerate(coef, start=1):
+        out += c * (np.roll(phi, -s_, axis=axis) - np.roll(phi, s_, axis=axis))
+    return out / (den * (box / m))
+
+
+def poisson_potential(delta_mesh, box: float, worder: int, lap_order: int, deconv_pow: int,
+                      coeff: float = 1.0, delta_mesh2=None):
+    """phi = IFFT(coeff * delta_hat / Lap / W~^deconv_pow), phi_hat(0) = 0 (O6 without the gradient)."""
+    d = np.asarray(delta_mesh, dtype=np.float64)
+    m = d.shape[0]
+    dh = _rfftn(d)
+    if delta_mesh2 is not None:
+        dh = 0.5 * (dh + interlace_phase_3d(m) * _rfftn(np.asarray(delta_mesh2, dtype=np.float64)))
+    delta = box / m
+    h = m // 2 + 1
+    l1 = lap_symbol_1d(m, lap_order)
+    lap = (l1[:, None, None] + l1[None, :, None] + l1[None, None, :h]) / delta ** 2
+    lap[0, 0, 0] = 1.0
+    green = coeff / lap
+    green[0, 0, 0] = 0.0
+    if deconv_pow:
+        W1 = window_1d(m, worder)
+        green = green / (W1[:, None, None] * W1[None, :, None] * W1[None, None, :h]) ** deconv_pow
+    return _irfftn(green * dh, m)
+
+
+def poisson_force_real_gradient(delta_mesh, box, worder, grad_order, lap_order, deconv_pow, coeff=1.0,
+                                delta_mesh2=None):
+    """g_a = -stencil_a(phi): the same operator as poisson_force for grad_order 2, 4, 6 (the Fourier
+    symbols of Table 2 are the DFTs of these stencils), evaluated with ONE inverse FFT."""
+    phi = poisson_potential(delta_mesh, box, worder, lap_order, deconv_pow, coeff, delta_mesh2)
+    return [-fd_gradient_real(phi, box, grad_order, a) for a in range(3)]
 
 
 # --------------------------------------------------------------------------------------

@@ -20,6 +20,9 @@ EXPORTED_SYMBOLS = (
 STAGE_NAMES = ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "interp", "vjp_scatter", "vjp_kspace", "vjp_gather")
 
 
+FLAG_BIN_TWOPASS, FLAG_NO_XFUSE, FLAG_GRAD_REAL, FLAG_KERNEL_GRAD = 1, 2, 4, 8  # pm_params.flags
+
+
 class PMError(RuntimeError):
     """A libpmforce call returned a negative pm_status."""
 
@@ -29,7 +32,7 @@ class _CParams(C.Structure):
         ("m", C.c_int32), ("worder", C.c_int32), ("interlace", C.c_int32), ("deconv_pow", C.c_int32),
         ("grad_order", C.c_int32), ("lap_order", C.c_int32), ("method", C.c_int32), ("nufft_width", C.c_int32),
         ("box", C.c_double), ("coeff", C.c_double), ("nufft_sigma", C.c_double), ("nufft_eps", C.c_double),
-        ("max_particles", C.c_int64),
+        ("max_particles", C.c_int64), ("flags", C.c_int32), ("reserved", C.c_int32),
     ]
 
 
@@ -49,11 +52,12 @@ class PMParams:
     nufft_sigma: float = 2.0
     nufft_eps: float = 1e-6
     nufft_width: int = 0
+    flags: int = 0  # FLAG_* bits (PM_FLAG_* of pmforce.h)
 
     def _c(self) -> _CParams:
         return _CParams(self.m, self.worder, self.interlace, self.deconv_pow, self.grad_order, self.lap_order,
                         self.method, self.nufft_width, self.box, self.coeff, self.nufft_sigma, self.nufft_eps,
-                        self.max_particles)
+                        self.max_particles, self.flags, 0)
 
 
 _lib = None

@@ -11,7 +11,7 @@ int need_method(Ctx* c, int method, const char* who) {
   if (!c) return PM_EINVAL;
   if (c->p.method != method)
     return fail(c, PM_ESTATE, "%s needs a ctx created with method = %d", who, method);
-  return PM_OK;
+  return enter_device(c);
 }
 
 ShiftSplit half_cell(const Ctx* c) {

@@ -1,14 +1,14 @@
 // pm_bin.cu -- a0: on-device counting sort of particles into mesh tiles (north_star: "Particles are
 // sorted into cell tiles with an on-device counting/Morton sort").  Not in the paper; the build's own step.
 //
-//   pass 1  k_count   : cell coordinate (fp64-accurate, see cell_coord) from the fp32 position, tile histogram
-//                       (warp-aggregated)
-//   scan    k_scan_*  : exclusive scans of the tile counts and of the per-tile work-item counts
-//   pass 2  k_permute : recompute the coordinate, claim a slot (warp-aggregated, order-preserving inside a
-//                       warp), store the record {ux, uy, uz, i} with tile-local fixed-point coordinates
-//   items   k_items   : work items (tile, begin, end) of at most ITEM_MAX particles (even split of dense tiles)
-//
-// Algorithmic bytes: 12N (read) + 12N (read) + 16N (write); the tile arrays are O(ntiles).
+// Default, single pass (k_bin_pass<2>): every tile owns a bucket of `capt` record slots (twice the mean load);
+//   one read of the positions: cell coordinate (fp64-accurate, see cell_coord), slot claim in the tile's bucket
+//   (warp-aggregated, order-preserving), record {ux, uy, uz, i} stored; claims beyond the bucket go to an
+//   overflow list that k_ov_permute sorts by tile behind the buckets.  k_scan_* scan the overflow counts and
+//   the work-item counts, k_items_bucketed writes the work items (tile, begin, end) of at most ITEM_MAX particles.
+//   12N read + 16N written.
+// PM_FLAG_BIN_TWOPASS (and N too large for 32-bit bucket indices): histogram (k_bin_pass<0>), scan, permute
+//   (k_bin_pass<1>), k_items: 12N + 12N read, 16N written, 16 B/particle of workspace instead of 68.
 #include "pm_internal.cuh"
 
 namespace pmf {

@@ -48,7 +48,14 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static EncodeTiledFn g_encode_tiled = nullptr;
 
-int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, bool swizzle128, CUtensorMap* out) {
+int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMap* out) {
+  for (int i = 0; i < c->ntmaps; ++i) {
+    const Ctx::TMapEntry& e = c->tmaps[i];
+    if (e.base == base && e.sx == sx && e.sy == sy && e.sz == sz) {
+      *out = e.map;
+      return PM_OK;
+    }
+  }
   if (!g_encode_tiled) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -64,10 +71,43 @@ int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, bool swizz
   const cuuint32_t box[3] = {(cuuint32_t)sz, (cuuint32_t)sy, (cuuint32_t)sx};
   const cuuint32_t estr[3] = {1, 1, 1};
   const CUresult r = g_encode_tiled(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(base), dims, strides,
-                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                    swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
-                                    (getenv("PMF_TMA_PROMO") ? (CUtensorMapL2promotion)atoi(getenv("PMF_TMA_PROMO")) : CU_TENSOR_MAP_L2_PROMOTION_L2_128B), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(c, PM_ECUDA, "cuTensorMapEncodeTiled failed: CUresult %d (box %d x %d x %d)", (int)r, sx, sy, sz);
+  constexpr int NT = (int)(sizeof(c->tmaps) / sizeof(c->tmaps[0]));
+  const int slot = c->ntmaps < NT ? c->ntmaps++ : (c->tmap_next++ % NT);  // full: overwrite round-robin
+  c->tmaps[slot].base = base;
+  c->tmaps[slot].sx = sx;
+  c->tmaps[slot].sy = sy;
+  c->tmaps[slot].sz = sz;
+  c->tmaps[slot].map = *out;
+  return PM_OK;
+}
+
+int kernel_occupancy(Ctx* c, const void* fn, int block, size_t smem, int* occ) {
+  for (int i = 0; i < c->nkern; ++i)
+    if (c->kern[i].fn == fn) {
+      *occ = c->kern[i].occ;
+      return PM_OK;
+    }
+  int o = 0;
+  PM_CUDA(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  PM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, fn, block, smem));
+  if (o < 1) return fail(c, PM_ECUDA, "kernel does not fit on an SM (%zu bytes of shared memory)", smem);
+  constexpr int NK = (int)(sizeof(c->kern) / sizeof(c->kern[0]));
+  if (c->nkern < NK) {
+    c->kern[c->nkern].fn = fn;
+    c->kern[c->nkern].occ = o;
+    ++c->nkern;
+  }
+  *occ = o;
+  return PM_OK;
+}
+
+int enter_device(Ctx* c) {
+  int dev = -1;
+  PM_CUDA(c, cudaGetDevice(&dev));
+  if (dev != c->device) PM_CUDA(c, cudaSetDevice(c->device));
   return PM_OK;
 }
 
@@ -185,6 +225,12 @@ static int validate(const pm_params& p, char* why, size_t n) {
       BAD("nufft_eps must be in (0, 1) when nufft_width = 0");
     if (p.interlace != 0) BAD("interlace is not defined for the NUFFT path");
   }
+  if (p.reserved != 0) BAD("reserved must be 0");
+  if (p.flags & ~(PM_FLAG_BIN_TWOPASS | PM_FLAG_NO_XFUSE | PM_FLAG_GRAD_REAL | PM_FLAG_KERNEL_GRAD))
+    BAD("unknown bit in flags");
+  if ((p.flags & PM_FLAG_GRAD_REAL) && (p.method != 0 || p.grad_order == 0))
+    BAD("PM_FLAG_GRAD_REAL needs method = 0 and grad_order 2, 4 or 6 (a finite-difference stencil of Table 2)");
+  if ((p.flags & PM_FLAG_KERNEL_GRAD) && p.method != 1) BAD("PM_FLAG_KERNEL_GRAD needs method = 1");
 #undef BAD
   return PM_OK;
 }
@@ -247,12 +293,11 @@ static int build(Ctx* c) {
   c->cap = p.max_particles;
   c->max_items = 2 * (int64_t)c->ntiles + c->cap / ITEM_MAX + 2;
   {  // single-pass binning: a bucket of twice the mean tile load per tile, overflow sorted behind the buckets
-    const char* e = getenv("PMF_BIN_TWOPASS");
     const int64_t mean = (c->cap + c->ntiles - 1) / c->ntiles;
     int64_t capt = (2 * mean + 31) / 32 * 32;
     if (capt < 64) capt = 64;
     const int64_t total = (int64_t)c->ntiles * capt + c->cap;
-    c->bin_capt = ((e && atoi(e) != 0) || total >= (int64_t)0xffffffff) ? 0u : (uint32_t)capt;
+    c->bin_capt = ((p.flags & PM_FLAG_BIN_TWOPASS) || total >= (int64_t)0xffffffff) ? 0u : (uint32_t)capt;
     c->ov_base = (uint32_t)((int64_t)c->ntiles * c->bin_capt);
   }
   const int scan_blocks = (c->ntiles + 4095) / 4096;

@@ -166,6 +166,19 @@ struct Ctx {
   int64_t launches;
   cudaStream_t prof_stream;
 
+  // per-ctx launch state (never process-wide statics: a second ctx may live on another device)
+  struct KernState {
+    const void* fn;
+    int occ;
+  } kern[96];        // kernels whose shared-memory attribute is set and whose occupancy is known
+  int nkern;
+  struct TMapEntry {
+    const float* base;
+    int sx, sy, sz;
+    CUtensorMap map;
+  } tmaps[24];       // tensor maps of the meshes the gather has staged (a mesh pointer + box identifies one)
+  int ntmaps, tmap_next;
+
   char err[512];
 };
 
@@ -209,10 +222,15 @@ inline GatherArgs gather_values(int ncomp, const float* const* mesh, float* out,
   return a;
 }
 int launch_gather(Ctx* c, int order, const ShiftSplit& sh, const GatherArgs& a, cudaStream_t st);
+// Sets cudaFuncAttributeMaxDynamicSharedMemorySize and returns the resident CTAs per SM of a kernel on this
+// ctx's device; both are done once per (ctx, kernel).
+int kernel_occupancy(Ctx* c, const void* fn, int block, size_t smem, int* occ);
+// The calls of include/pmforce.h run on the device the ctx was created on.
+int enter_device(Ctx* c);
 // Tensor map of a dense fp32 [m][m][m] mesh (m = c->mg) with a box of sx * sy * sz elements, no swizzle,
 // out-of-bounds elements zero-filled.  base must be 16-byte aligned (PM_EINVAL otherwise).
-// swizzle128: the box rows (sz * 4 = 128 bytes) land in shared memory with TMA's 128-byte swizzle
-int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, bool swizzle128, CUtensorMap* out);
+// Encoded once per (mesh pointer, box) and kept in the ctx.
+int make_mesh_tmap(Ctx* c, const float* base, int sx, int sy, int sz, CUtensorMap* out);
 
 // NUFFT spreading / interpolation with the ES kernel (same conventions).
 int launch_es_scatter(Ctx* c, int ncomp, const float* wsrc, int wstride, float* const mesh[],

@@ -10,7 +10,6 @@
 //            P^3 nodes from there.
 #pragma once
 #include <cuda.h>
-#include <stdlib.h>
 
 #include "pm_internal.cuh"
 
@@ -714,25 +713,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   } while (!ok);
 }
 // box (innermost first) at coordinates (c0, c1, c2) = (z, y, x); out-of-bounds elements are zero-filled
-__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
-                                            uint64_t policy) {
-  if (policy == 0) {
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
-        : "memory");
-    return;
-  }
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2) {
   asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
-      " [%0], [%1, {%3, %4, %5}], [%2], %6;"
-      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2)
       : "memory");
-}
-__device__ __forceinline__ uint64_t l2_policy_evict_last() {
-  uint64_t p;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-  return p;
 }
 
 // ---- K4 / K7: tile gather ----------------------------------------------------------------------------
@@ -742,7 +727,7 @@ __device__ __forceinline__ uint64_t l2_policy_evict_last() {
 //
 // Persistent CTAs draw work items from the dynamic schedule.  Thread 0 stages the tile + halo box of every
 // component with one TMA tensor copy each (north_star "TMA staging of mesh tiles"), completion on an
-// mbarrier, L2 evict-last hint (the halo planes are read again by the neighbouring tiles); with STAGES = 2
+// mbarrier (an L2 evict-last hint on the copies was measured and changed nothing); with STAGES = 2
 // the box of the CTA's next item is in flight while the particles of the current one are interpolated.
 // TMA zero-fills what lies beyond the mesh edge, it does not wrap: tiles whose box crosses an edge (a few
 // per cent) are patched by the threads with periodic loads after the copy has landed.  roll in [0, m); when
@@ -768,13 +753,11 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
 
-  uint64_t policy = 0;
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < STAGES; ++s) mbar_init(&s_bar[s], 1);
     fence_barrier_init();
     fence_proxy_async();
-    if (manual >> 1) policy = l2_policy_evict_last();
     s_next[0] = sched_next(bv.sched);  // the item after this CTA's first
   }
   __syncthreads();
@@ -793,8 +776,8 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
     for (int a = 0; a < NCOMP; ++a) {  // main plane (first TZ nodes of every row) and halo plane (the rest)
       float* dst = s_base + (stage * NCOMP + a) * G::COMP;
-      tma_load_3d(dst, &maps.m[2 * a], &s_bar[stage], cz, cy, cx, policy);
-      tma_load_3d(dst + G::MAIN, &maps.m[2 * a + 1], &s_bar[stage], cz + TZ, cy, cx, policy);
+      tma_load_3d(dst, &maps.m[2 * a], &s_bar[stage], cz, cy, cx);
+      tma_load_3d(dst + G::MAIN, &maps.m[2 * a + 1], &s_bar[stage], cz + TZ, cy, cx);
     }
   };
 
@@ -842,10 +825,11 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         group_pos<G>(rr, row, zoff);
         const int sy = row % G::SY, sx = row / G::SY;
         if (!(manual & 1) && cx + sx < m && cy + sy < m && cz + zoff + 3 < m) continue;  // TMA delivered it
-        const float* p = mesh.p[comp] + ((size_t)wrap_hi(cx + sx, m) * m + wrap_hi(cy + sy, m)) * m;
+        // true modulo: on the smallest meshes (m < 24) the box is longer than two periods of the mesh
+        const float* p = mesh.p[comp] + ((size_t)((cx + sx) % m) * m + (cy + sy) % m) * m;
         const int gz = cz + zoff;
-        const float4 v = make_float4(__ldg(p + wrap_hi(gz, m)), __ldg(p + wrap_hi(gz + 1, m)),
-                                     __ldg(p + wrap_hi(gz + 2, m)), __ldg(p + wrap_hi(gz + 3, m)));
+        const float4 v = make_float4(__ldg(p + gz % m), __ldg(p + (gz + 1) % m), __ldg(p + (gz + 2) % m),
+                                     __ldg(p + (gz + 3) % m));
         reinterpret_cast<float4*>(s_w + comp * G::COMP)[rr] = v;
       }
       fence_proxy_async();  // generic-proxy writes before the async proxy refills this buffer
@@ -945,10 +929,6 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 }
 
 // ---- host-side launch helpers ------------------------------------------------------------------------
-inline int tune_flag(const char* name, int dflt) {  // tuning knobs read once from the environment
-  const char* v = getenv(name);
-  return v ? atoi(v) : dflt;
-}
 inline int norm_roll(int r, int m) {
   r %= m;
   return r < 0 ? r + m : r;
@@ -969,12 +949,8 @@ int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const f
   constexpr int NBUF = 2 * acc_bytes <= 48 * 1024 ? 2 : 1;  // two accumulator tiles when they are cheap
   const size_t smem = NBUF * acc_bytes;
   auto kern = k_scatter<T, NCOMP, WEIGHTED, NBUF>;
-  static int occ = 0;
-  if (!occ) {
-    PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    PM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLOCK, smem));
-    if (occ < 1) return fail(c, PM_ECUDA, "scatter kernel does not fit on an SM");
-  }
+  int occ = 0;
+  PM_TRY(kernel_occupancy(c, (const void*)kern, BLOCK, smem, &occ));
   MeshPtrs<NCOMP> mp;
   for (int a = 0; a < NCOMP; ++a) mp.p[a] = mesh[a];
   const int m = c->mg;
@@ -989,18 +965,12 @@ int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const f
 // Unit-weight, single-field scatter with warp-private tiles (k_scatter_warp).
 template <class T>
 int run_scatter_warp(Ctx* c, const typename T::Params& tp, const int roll[3], float* mesh, cudaStream_t st) {
-  static const bool use_stores = tune_flag("PMF_SCATTER_STORES", 1) != 0;  // A/B switch for measurements
-  const int zeroed = (use_stores && c->scatter_mesh_zeroed) ? 1 : 0;
+  const int zeroed = c->scatter_mesh_zeroed ? 1 : 0;
   using G = Geo<T>;
   constexpr size_t smem = sizeof(int) * (size_t)WS_WARPS * G::COMP;
-  static const bool fast = tune_flag("PMF_SCATTER_FASTCIC", 1) != 0;  // A/B switch for measurements
-  auto kern = fast ? k_scatter_warp<T, true> : k_scatter_warp<T, false>;
-  static int occ = 0;
-  if (!occ) {
-    PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    PM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, WS_WARPS * 32, smem));
-    if (occ < 1) return fail(c, PM_ECUDA, "scatter kernel does not fit on an SM");
-  }
+  auto kern = k_scatter_warp<T, true>;
+  int occ = 0;
+  PM_TRY(kernel_occupancy(c, (const void*)kern, WS_WARPS * 32, smem, &occ));
   const int64_t bound = ((int64_t)c->ntiles + c->bin_n / ITEM_MAX + 1 + WS_WARPS - 1) / WS_WARPS;
   const int64_t cap = (int64_t)c->num_sms * occ;
   const int m = c->mg;
@@ -1020,24 +990,20 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const fl
   constexpr int STAGES = 2 * stage_bytes <= 100 * 1024 ? 2 : 1;
   constexpr size_t smem = STAGES * stage_bytes + 128;
   auto kern = k_gather<T, NCOMP, GRAD, STAGES>;
-  static int occ = 0;
-  if (!occ) {
-    PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    PM_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, BLOCK, smem));
-    if (occ < 1) return fail(c, PM_ECUDA, "gather kernel does not fit on an SM");
-  }
+  int occ = 0;
+  PM_TRY(kernel_occupancy(c, (const void*)kern, BLOCK, smem, &occ));
   CMeshPtrs<NCOMP> mp;
   TMapSet<2 * NCOMP> maps;
   const int m = c->mg;
   for (int a = 0; a < NCOMP; ++a) {
     mp.p[a] = mesh[a];
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, false, &maps.m[2 * a]));
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::HZ, false, &maps.m[2 * a + 1]));
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, &maps.m[2 * a]));
+    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::HZ, &maps.m[2 * a + 1]));
   }
   const float a_eff = GRAD ? (float)((double)alpha * (double)c->mg / c->p.box) : alpha;
   const int3 nr = make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m));
   kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp, nr, maps, mp, cot, cstride, ncot, const_coef, wmul,
-                                               a_eff, accumulate ? 1 : 0, ((nr.z & 3) ? 1 : 0) | (tune_flag("PMF_TMA_EVICT_LAST", 0) << 1), out);
+                                               a_eff, accumulate ? 1 : 0, (nr.z & 3) ? 1 : 0, out);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

@@ -12,15 +12,11 @@ static int scatter_os(Ctx* c, const ShiftSplit& sh, int ncomp, const float* wsrc
   for (int a = 0; a < 3; ++a) tp.frac[a] = sh.frac[a];
   if (!wsrc) {  // unit weights: every component receives the same field
     // CIC: four warp-private accumulator tiles per CTA fit four CTAs on an SM -> the barrier-free kernel
-    static const bool coop = tune_flag("PMF_SCATTER_COOP", 0) != 0;  // A/B switch for measurements
     for (int a = 0; a < ncomp; ++a) {
-      if constexpr (ORDER == 2) {
-        if (!coop) {
-          PM_TRY((run_scatter_warp<T>(c, tp, sh.roll, mesh[a], st)));
-          continue;
-        }
-      }
-      PM_TRY((run_scatter<T, 1, false>(c, tp, sh.roll, nullptr, 0, mesh + a, st)));
+      if constexpr (ORDER == 2)
+        PM_TRY((run_scatter_warp<T>(c, tp, sh.roll, mesh[a], st)));
+      else
+        PM_TRY((run_scatter<T, 1, false>(c, tp, sh.roll, nullptr, 0, mesh + a, st)));
     }
     return PM_OK;
   }

@@ -365,8 +365,7 @@ bool xfft_supported(int m) { return m == 64 || m == 128 || m == 256 || m == 512 
 int xfft_init(Ctx* c) {  // twiddle table and the batched 2-D (y,z) cuFFT plans; called from pm_create
   c->xfused = false;
   if (!xfft_supported(c->mg)) return PM_OK;
-  const char* off = getenv("PMF_NO_XFUSE");  // A/B switch for measurements and for testing the unfused path
-  if (off && atoi(off)) return PM_OK;
+  if (c->p.flags & PM_FLAG_NO_XFUSE) return PM_OK;
   const int m = c->mg;
   std::vector<float2> tw(m);
   for (int k = 0; k < m; ++k) {
@@ -425,11 +424,8 @@ static int xfft_launch_n(Ctx* c, const XTabs& t, const float2* i0, const float2*
   constexpr int NT = N * XC / XEPT;
   constexpr size_t smem = sizeof(float2) * 2 * (size_t)xfft_smem_elems<N>();
   auto kern = k_xfft_kspace<N, MODE>;
-  static bool attr = false;
-  if (!attr) {
-    PM_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr = true;
-  }
+  int occ = 0;
+  PM_TRY(kernel_occupancy(c, (const void*)kern, NT, smem, &occ));
   const int64_t grid = (t.ncol + XC - 1) / XC;
   kern<<<(unsigned)grid, NT, smem, st>>>(t, i0, i1, i2, o0, o1, o2, coeff_eff);
   count_launch(c);

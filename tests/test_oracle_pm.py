@@ -195,3 +195,83 @@ def test_deconvolution_divides_by_window_power():
     for p in (1, 2):
         win = np.prod(np.sinc(n0 / m) ** 3)
         assert np.abs(po.poisson_force(np.cos(phase), box, 3, 4, 0, p)[0] - base / win ** p).max() < 1e-12
+
+
+# ---------------------------------------------------------------- forward-mode rules, Eq. C.13
+@pytest.mark.parametrize("worder", (3, 4))
+@pytest.mark.parametrize("shifted", (False, True))
+def test_jvp_rules_match_central_differences(worder, shifted):
+    """Eq. C.13a/b (:943-945): tangents of scatter and gather w.r.t. positions, weights and mesh against
+    central differences of Eq. C.1 / C.2 (TSC / PCS: continuous derivatives)."""
+    m, box, n = 10, 25.0, 200
+    rng = np.random.default_rng(40 + worder)
+    pos = uniform_random(n, box, 41).astype(np.float64)
+    w = rng.standard_normal(n)
+    tX, tw = rng.standard_normal((n, 3)), rng.standard_normal(n)
+    mesh, tmesh = rng.standard_normal((m, m, m)), rng.standard_normal((m, m, m))
+    rho_in_tan = rng.standard_normal((m, m, m))
+    shift = np.array([0.3, -1.7, 0.5 * box / m]) if shifted else None
+    h = 1e-6
+    fd = (po.scatter(pos + h * tX, m, box, worder, weights=w + h * tw, shift=shift)
+          - po.scatter(pos - h * tX, m, box, worder, weights=w - h * tw, shift=shift)) / (2 * h) + rho_in_tan
+    jvp = po.scatter_jvp(pos, m, box, worder, weights=w, pos_tan=tX, w_tan=tw, shift=shift, mesh_tan=rho_in_tan)
+    assert np.abs(fd - jvp).max() < 1e-7 * np.abs(jvp).max()
+    fdg = (po.gather(mesh + h * tmesh, pos + h * tX, box, worder, shift=shift)
+           - po.gather(mesh - h * tmesh, pos - h * tX, box, worder, shift=shift)) / (2 * h)
+    jg = po.gather_jvp(mesh, pos, box, worder, pos_tan=tX, mesh_tan=tmesh, shift=shift)
+    assert np.abs(fdg - jg).max() < 1e-7 * np.abs(jg).max()
+
+
+@pytest.mark.parametrize("worder", ORDERS)
+def test_jvp_vjp_duality(worder):
+    """<JVP(tangent), cotangent> = <tangent, VJP(cotangent)> for scatter and gather (rule table :949-960);
+    also pins the CIC rules, whose derivative is piecewise constant (R12)."""
+    m, box, n = 9, 18.0, 150
+    rng = np.random.default_rng(50 + worder)
+    pos = uniform_random(n, box, 51)
+    w = rng.standard_normal(n)
+    tX, tw = rng.standard_normal((n, 3)), rng.standard_normal(n)
+    cot_mesh = rng.standard_normal((m, m, m))
+    lhs = np.sum(po.scatter_jvp(pos, m, box, worder, weights=w, pos_tan=tX, w_tan=tw) * cot_mesh)
+    xbar = np.stack([w * po.gather(cot_mesh, pos, box, worder, deriv_axis=a) for a in range(3)], axis=1)  # Eq. C.6
+    wbar = po.gather(cot_mesh, pos, box, worder)                                                          # Eq. C.8
+    assert abs(lhs - (np.sum(tX * xbar) + np.sum(tw * wbar))) < 1e-11 * max(1.0, abs(lhs))
+    mesh, tmesh = rng.standard_normal((m, m, m)), rng.standard_normal((m, m, m))
+    cot_v = rng.standard_normal(n)
+    lhs = np.sum(po.gather_jvp(mesh, pos, box, worder, pos_tan=tX, mesh_tan=tmesh) * cot_v)
+    mbar = po.scatter(pos, m, box, worder, weights=cot_v)                                                 # Eq. C.10
+    xbar = np.stack([cot_v * po.gather(mesh, pos, box, worder, deriv_axis=a) for a in range(3)], axis=1)  # Eq. C.12
+    assert abs(lhs - (np.sum(tmesh * mbar) + np.sum(tX * xbar))) < 1e-11 * max(1.0, abs(lhs))
+
+
+# ---------------------------------------------------------------- Table 2, "Real" column
+def test_real_space_stencils_are_the_printed_ones(golden_dir):
+    for kind, order, den, *coef in _load_table(os.path.join(golden_dir, "table2_stencils.txt")):
+        if kind != "grad":
+            continue
+        d, c = po.GRAD_STENCIL[int(order)]
+        r = len(c)
+        printed = [float(v) for v in coef]
+        assert d == float(den) and printed[r] == 0.0
+        assert printed[r + 1:] == list(c) and printed[:r] == [-v for v in reversed(c)]
+
+
+@pytest.mark.parametrize("order", (2, 4, 6))
+@pytest.mark.parametrize("interlaced", (False, True))
+def test_real_space_gradient_equals_fourier_symbol(order, interlaced):
+    """g = -stencil(IFFT(phi_hat)) is the same operator as IFFT(-i D(theta)/Delta phi_hat) (Table 2: the
+    Fourier entries are the DFTs of the stencils): one inverse FFT instead of three."""
+    m, box = 12, 30.0
+    d = np.random.default_rng(60).standard_normal((2, m, m, m))
+    d2 = d[1] if interlaced else None
+    a = po.poisson_force(d[0], box, 3, order, 0, 2, coeff=1.3, delta_mesh2=d2)
+    b = po.poisson_force_real_gradient(d[0], box, 3, order, 0, 2, coeff=1.3, delta_mesh2=d2)
+    for x, y in zip(a, b):
+        assert np.abs(x - y).max() < 1e-13 * np.abs(x).max()
+    # the stencil differentiates a resolved plane wave to its order of accuracy
+    x = np.arange(m) * (box / m)
+    f = np.broadcast_to(np.sin(2 * np.pi * x / box)[:, None, None], (m, m, m))
+    exact = np.broadcast_to((2 * np.pi / box) * np.cos(2 * np.pi * x / box)[:, None, None], (m, m, m))
+    err = np.abs(po.fd_gradient_real(f, box, order, 0) - exact).max() / (2 * np.pi / box)
+    assert err < {2: 0.05, 4: 4e-3, 6: 4e-4}[order]
+    assert np.abs(po.fd_gradient_real(f, box, order, 1)).max() < 1e-14

@@ -174,6 +174,23 @@ def _kspace_multiplier(m_fine: int, m: int, box: float, n_particles: int, w: int
     return [1j * ka * base for ka in (kx, ky, kz)]
 
 
+def kspace_multiplier_at(idx, m_fine: int, m: int, box: float, n_particles: int, w: int, beta: float,
+                         coeff: float):
+    """M_a(n) of :func:`_kspace_multiplier` for single modes idx = (ix, iy, iz) (FFT indices on the fine
+    grid, arrays allowed); complex [3, ...].  For fine grids too large for the 3-D arrays; pinned against
+    _kspace_multiplier element by element."""
+    ix, iy, iz = (np.asarray(v, dtype=np.int64) for v in idx)
+    nf = np.fft.fftfreq(m_fine, 1.0 / m_fine)
+    keep = np.abs(nf) < 0.5 * m
+    ph1 = es_kernel_ft(nf, m_fine, w, beta)
+    k1 = (2.0 * np.pi / box) * nf
+    k2 = k1[ix] ** 2 + k1[iy] ** 2 + k1[iz] ** 2
+    ok = keep[ix] & keep[iy] & keep[iz] & (k2 > 0.0)
+    phat = ph1[ix] * ph1[iy] * ph1[iz]
+    base = np.where(ok, (coeff / n_particles) / (np.where(ok, k2, 1.0) * phat * phat), 0.0)
+    return np.stack([1j * k1[i] * base for i in (ix, iy, iz)])
+
+
 def nufft_kspace(fine, m: int, box: float, n_particles: int, w: int, beta: float, coeff: float = 1.0):
     """Spread grid -> three fine force grids ready for ``es_interp`` (:260-264)."""
     fine = np.asarray(fine, dtype=np.float64)

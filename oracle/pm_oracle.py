@@ -311,6 +311,24 @@ def force_symbols(m: int, box: float, worder: int, grad_order: int, lap_order: i
     return S
 
 
+def force_symbol_at(idx, m: int, box: float, worder: int, grad_order: int, lap_order: int,
+                    deconv_pow: int, coeff: float):
+    """S_a(n) of :func:`force_symbols` for single modes: idx = (ix, iy, iz) integer FFT indices in [0, m)
+    (arrays allowed); returns complex [3, ...].  For meshes too large to hold the 3-D symbol arrays
+    (m = 1024); pinned against force_symbols element by element."""
+    ix, iy, iz = (np.asarray(v, dtype=np.int64) for v in idx)
+    delta = box / m
+    D = grad_symbol_1d(m, grad_order)
+    l1 = lap_symbol_1d(m, lap_order)
+    W1 = window_1d(m, worder)
+    lap = (l1[ix] + l1[iy] + l1[iz]) / delta ** 2
+    zero = (ix == 0) & (iy == 0) & (iz == 0)
+    green = np.where(zero, 0.0, coeff / np.where(zero, 1.0, lap))
+    if deconv_pow:
+        green = green / (W1[ix] * W1[iy] * W1[iz]) ** deconv_pow
+    return np.stack([-(1j * D[i] / delta) * green for i in (ix, iy, iz)])
+
+
 def interlace_phase(m: int):
     """Per-axis factor of e^{-i k.s} for s = (Delta/2)(1,1,1): exp(-i pi n_a/m); reading R9:
     real part only (= 0) on the Nyquist index so the combined field stays Hermitian."""

@@ -34,4 +34,8 @@ from .api import (  # noqa: F401
     library_path,
     load_library,
     EXPORTED_SYMBOLS,
+    FLAG_BIN_TWOPASS,
+    FLAG_NO_XFUSE,
+    FLAG_GRAD_REAL,
+    FLAG_KERNEL_GRAD,
 )

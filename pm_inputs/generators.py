@@ -213,3 +213,38 @@ def make_config_positions(name: str, n_p: int | None = None, m: int | None = Non
         if shuffle:
             pos = pos[np.random.default_rng(c["seed"] + 1).permutation(pos.shape[0])]
     return pos, c
+
+
+def plane_wave_modes(m: int, n_waves: int, seed: int):
+    """Seeded set of distinct Fourier modes and complex amplitudes for a synthetic mesh field
+    f(j) = Re sum_w c_w exp(2 pi i n_w . j / m): integer FFT indices idx [W, 3] in [0, m) and c [W].
+    Mixes low wave numbers, modes on the Nyquist planes and modes with zero components with random ones;
+    no mode is its own conjugate and no two modes are conjugates of each other."""
+    rng = np.random.default_rng(seed)
+    idx = rng.integers(0, m, size=(n_waves, 3))
+    k = n_waves // 8
+    idx[:k] = rng.integers(-3, 4, size=(k, 3)) % m                      # low |n|
+    idx[k:2 * k, rng.integers(0, 3)] = m // 2                           # a Nyquist plane
+    idx[2 * k:3 * k, 0] = 0                                             # n_x = 0 plane
+    idx[3 * k:4 * k, 2] = rng.integers(0, 2, size=k) * (m // 2)         # n_z in {0, Nyquist}
+    seen, keep = set(), []
+    for w in range(n_waves):
+        t = tuple(int(v) for v in idx[w])
+        neg = tuple((-v) % m for v in t)
+        if t == neg or t in seen or neg in seen:
+            continue
+        seen.add(t)
+        keep.append(w)
+    idx = idx[keep]
+    coef = rng.standard_normal(len(keep)) + 1j * rng.standard_normal(len(keep))
+    return idx, coef
+
+
+def plane_wave_values(m: int, idx, coef, nodes):
+    """f at integer node triples ``nodes`` [K, 3] for the field of :func:`plane_wave_modes`, fp64."""
+    nodes = np.asarray(nodes, dtype=np.int64)
+    out = np.zeros(nodes.shape[0])
+    for w0 in range(0, idx.shape[0], 64):  # chunks keep the phase table small
+        ph = (nodes @ idx[w0:w0 + 64].T.astype(np.int64)) % m
+        out += (np.exp(2j * np.pi * ph / m) * coef[None, w0:w0 + 64]).real.sum(axis=1)
+    return out

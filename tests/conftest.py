@@ -16,14 +16,3 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def golden_dir():
     return os.path.join(ROOT, "tests", "golden")
-
-
-def record_error(name: str, value: float, tol: float):
-    """Append a measured parity error to gpurun_out/parity_errors.tsv (kept beside the GPU test log)."""
-    out = os.path.join(ROOT, "gpurun_out")
-    try:
-        os.makedirs(out, exist_ok=True)
-        with open(os.path.join(out, "parity_errors.tsv"), "a") as f:
-            f.write(f"{name}\t{value:.3e}\t{tol:.1e}\n")
-    except OSError:
-        pass

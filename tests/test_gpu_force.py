@@ -12,7 +12,7 @@ from oracle import nufft_oracle as no
 from oracle import pm_oracle as po
 from pm_inputs import generators as gen
 
-from conftest import record_error
+from parity_util import check, record_error, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -27,12 +27,6 @@ def pm():
     import paper_2510_05206_b200 as pm_
 
     return pm_
-
-
-def rel_l2(a, b):
-    a = np.asarray(a, dtype=np.float64)
-    b = np.asarray(b, dtype=np.float64)
-    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
 def dev(x):
@@ -81,9 +75,7 @@ def test_force_parity_configs(pm, name, n_p, shuffle):
     pos, c = gen.make_config_positions(name, n_p=n_p, shuffle=shuffle)
     f = gpu_force(pm, params_of(pm, c, pos.shape[0]), pos)
     ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
-    err = rel_l2(f, ref)
-    record_error(f"force/{name}/n_p={n_p or c['n_p']}/shuffle={int(shuffle)}", err, FORCE_TOL)
-    assert err <= FORCE_TOL, err
+    check(f"force/{name}/n_p={n_p or c['n_p']}/shuffle={int(shuffle)}", f, ref, FORCE_TOL)
     if c.get("interlace", 0) != 1:  # momentum conservation (same W for assign and gather); not for R1 mode 1
         assert np.abs(f.astype(np.float64).sum(axis=0)).max() <= 2e-6 * np.abs(f).sum()
 
@@ -95,9 +87,7 @@ def test_force_parity_kernels_and_interlacing(pm, worder, interlace):
     c = dict(c, worder=worder, interlace=interlace)
     f = gpu_force(pm, params_of(pm, c, pos.shape[0]), pos)
     ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
-    err = rel_l2(f, ref)
-    record_error(f"force/cfg1-48/worder={worder}/interlace={interlace}", err, FORCE_TOL)
-    assert err <= FORCE_TOL, err
+    check(f"force/cfg1-48/worder={worder}/interlace={interlace}", f, ref, FORCE_TOL)
 
 
 @pytest.mark.parametrize("m", [24, 40, 72])
@@ -117,9 +107,7 @@ def test_force_parity_ragged_tiles(pm, m, interlace):
     c = dict(m=m, box=box, worder=2, interlace=interlace, grad_order=4, lap_order=0, deconv_pow=2)
     f = gpu_force(pm, params_of(pm, c, n), pos)
     ref = po.force(pos, m, box, **oracle_kw(c))
-    err = rel_l2(f, ref)
-    record_error(f"force/ragged-m={m}/interlace={interlace}", err, FORCE_TOL)
-    assert err <= FORCE_TOL, err
+    check(f"force/ragged-m={m}/interlace={interlace}", f, ref, FORCE_TOL)
 
 
 def test_zero_force_on_lattice(pm):
@@ -142,9 +130,7 @@ def test_force_vjp_parity(pm, name, n_p, interlace):
     lam = gen.gaussian_cotangent(pos.shape[0], c.get("cot_seed", 2000))
     xb = gpu_force_vjp(pm, params_of(pm, c, pos.shape[0]), pos, lam)
     ref = po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c))
-    err = rel_l2(xb, ref)
-    record_error(f"force_vjp/{name}/n_p={n_p or c['n_p']}/interlace={interlace}", err, VJP_TOL)
-    assert err <= VJP_TOL, err
+    check(f"force_vjp/{name}/n_p={n_p or c['n_p']}/interlace={interlace}", xb, ref, VJP_TOL)
 
 
 def test_force_vjp_parity_cfg1_full(pm):
@@ -153,9 +139,7 @@ def test_force_vjp_parity_cfg1_full(pm):
     lam = gen.gaussian_cotangent(pos.shape[0], c["cot_seed"])
     xb = gpu_force_vjp(pm, params_of(pm, c, pos.shape[0]), pos, lam)
     ref = po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c))
-    err = rel_l2(xb, ref)
-    record_error("force_vjp/cfg1/full", err, VJP_TOL)
-    assert err <= VJP_TOL, err
+    check("force_vjp/cfg1/full", xb, ref, VJP_TOL)
 
 
 # ---- NUFFT path -----------------------------------------------------------------------------------------
@@ -177,19 +161,42 @@ def test_nufft_stage_parity(pm, width):
     fine = torch.zeros(mf, mf, mf, device="cuda")
     pm.nufft_spread(ctx, dev(pos), dev(c), fine)
     ref = no.es_spread(pos, mf, box, w, beta, weights=c)
-    assert rel_l2(fine.cpu().numpy(), ref) <= 2e-6
+    check("fine", fine, ref, 2e-6)
     meshes = gen.random_mesh(mf, 17, 3)
     out = torch.empty(n, 3, device="cuda")
     pm.nufft_interp(ctx, [dev(meshes[a]) for a in range(3)], dev(pos), out)
     refi = np.stack([no.es_interp(meshes[a], pos, box, w, beta) for a in range(3)], axis=1)
-    assert rel_l2(out.cpu().numpy(), refi) <= 2e-6
+    check("out", out, refi, 2e-6)
     # VJP pieces: grad gather (spread w.r.t. positions) and value gather (w.r.t. strengths)
     pc = torch.empty(n, 3, device="cuda")
     cc = torch.empty(n, device="cuda")
     pm.nufft_spread_vjp(ctx, dev(pos), dev(c), dev(meshes[0]), pos_cot=pc, c_cot=cc)
     refp = np.stack([c * no.es_interp(meshes[0], pos, box, w, beta, deriv_axis=b) for b in range(3)], axis=1)
-    assert rel_l2(cc.cpu().numpy(), refi[:, 0]) <= 2e-6
-    assert rel_l2(pc.cpu().numpy(), refp) <= 5e-6
+    check("cc", cc, refi[:, 0], 2e-6)
+    check("pc", pc, refp, 5e-6)
+    pm.pm_destroy(ctx)
+
+
+@pytest.mark.parametrize("width,ncomp", [(4, 3), (7, 1), (7, 3), (8, 2)])
+def test_nufft_interp_vjp_parity(pm, width, ncomp):
+    """nufft_interp_vjp: the scatter of the cotangents with the ES kernel (Eq. C.10) and the grad-kernel gather
+    weighted by them (Eq. C.12), App. C with W -> ES kernel (:858)."""
+    m, box = 20, 50.0
+    pos = np.concatenate([gen.uniform_random(12000, box, 64), gen.lattice_displaced(16, 40, box, 2.0, 65)])
+    n = pos.shape[0]
+    ctx = pm.pm_create(nufft_params(pm, m, box, n, width=width))
+    mf, w, beta = ctx.mg, ctx.nufft_width, ctx.nufft_beta
+    meshes = gen.random_mesh(mf, 18, ncomp)
+    cot = gen.gaussian_cotangent(n, 66, ncomp)
+    fc = [torch.zeros(mf, mf, mf, device="cuda") for _ in range(ncomp)]
+    pc = torch.empty(n, 3, device="cuda")
+    pm.nufft_interp_vjp(ctx, [dev(meshes[a]) for a in range(ncomp)], dev(pos), dev(cot), fine_cot=fc, pos_cot=pc)
+    refp = np.zeros((n, 3))
+    for a in range(ncomp):
+        check(f"fine_cot{a}", fc[a], no.es_spread(pos, mf, box, w, beta, weights=cot[:, a]), 5e-6)
+        for b in range(3):
+            refp[:, b] += cot[:, a] * no.es_interp(meshes[a], pos, box, w, beta, deriv_axis=b)
+    check("pos_cot", pc, refp, 5e-6)
     pm.pm_destroy(ctx)
 
 
@@ -202,12 +209,12 @@ def test_nufft_kspace_parity(pm):
     pm.nufft_poisson_force(ctx, dev(fine), n, g)
     ref = no.nufft_kspace(fine, m, box, n, w, beta)
     for a in range(3):
-        assert rel_l2(g[a].cpu().numpy(), ref[a]) <= 3e-6
+        check("g[a]", g[a], ref[a], 3e-6)
     cot = gen.random_mesh(mf, 20, 3)
     fc = torch.empty(mf, mf, mf, device="cuda")
     pm.nufft_poisson_force_vjp(ctx, [dev(cot[a]) for a in range(3)], n, fc)
     refv = no.nufft_kspace_vjp([cot[a] for a in range(3)], m, box, n, w, beta)
-    assert rel_l2(fc.cpu().numpy(), refv) <= 3e-6
+    check("fc", fc, refv, 3e-6)
     pm.pm_destroy(ctx)
 
 
@@ -217,9 +224,7 @@ def test_nufft_force_vs_bruteforce_definition(pm):
     pos = gen.uniform_random(700, box, 63)
     f = gpu_force(pm, nufft_params(pm, m, box, pos.shape[0]), pos)
     ref = no.nudft_force_bruteforce(pos, m, box)
-    err = rel_l2(f, ref)
-    record_error("nufft_force/bruteforce-700", err, 1e-5)
-    assert err <= 1e-5, err
+    check("nufft_force/bruteforce-700", f, ref, 1e-5)
 
 
 @pytest.mark.parametrize("sigma,eps,width", [(2.0, 1e-6, 0), (1.25, 1e-4, 0), (2.0, 1e-3, 0), (1.25, 0.5, 5)])
@@ -229,9 +234,7 @@ def test_nufft_force_parity(pm, sigma, eps, width):
     pos, c = gen.make_config_positions("cfg3", n_p=48)
     f = gpu_force(pm, nufft_params(pm, c["m"], c["box"], pos.shape[0], sigma=sigma, eps=eps, width=width), pos)
     ref = no.nufft_force(pos, c["m"], c["box"], sigma=sigma, eps=eps, width=width)
-    err = rel_l2(f, ref)
-    record_error(f"nufft_force/cfg3-48/sigma={sigma}/eps={eps}/w={width}", err, 1e-5)
-    assert err <= 1e-5, err
+    check(f"nufft_force/cfg3-48/sigma={sigma}/eps={eps}/w={width}", f, ref, 1e-5)
 
 
 def test_nufft_force_vjp_parity(pm):
@@ -239,9 +242,7 @@ def test_nufft_force_vjp_parity(pm):
     lam = gen.gaussian_cotangent(pos.shape[0], 2003)
     xb = gpu_force_vjp(pm, nufft_params(pm, c["m"], c["box"], pos.shape[0]), pos, lam)
     ref = no.nufft_force_vjp(pos, lam, c["m"], c["box"])
-    err = rel_l2(xb, ref)
-    record_error("nufft_force_vjp/cfg3-32", err, VJP_TOL)
-    assert err <= VJP_TOL, err
+    check("nufft_force_vjp/cfg3-32", xb, ref, VJP_TOL)
 
 
 def test_pm_force_host_matches_device(pm):
@@ -253,32 +254,10 @@ def test_pm_force_host_matches_device(pm):
     fh = torch.empty(pos.shape[0], 3).pin_memory()
     pm.pm_force_host(ctx, ph, fh)
     ref = po.force(pos, c["m"], c["box"], **oracle_kw(c))
-    assert rel_l2(fh.numpy(), ref) <= FORCE_TOL
-    assert rel_l2(fh.numpy(), f_dev.cpu().numpy()) <= 2e-6  # atomics: not bitwise
+    check("host_vs_oracle", fh.numpy(), ref, FORCE_TOL)
+    check("host_vs_device", fh.numpy(), f_dev.cpu().numpy(), 2e-6)  # atomics: not bitwise
     pm.pm_set_profiling(ctx, True)
     pm.pm_force(ctx, dev(pos), f_dev)
     ms, launches = pm.pm_get_stage_ms(ctx)
     assert launches >= 8 and ms["assign"] > 0 and ms["interp"] > 0
     pm.pm_destroy(ctx)
-
-
-def test_force_parity_headline_full_size_sampled(pm):
-    """The bench workload itself (N = 512^3 particles, 512^3 mesh, the launch configuration bench.py times):
-    the oracle assigns all particles and solves for the three force meshes at full size in fp64, then
-    interpolates them for a seeded sample of particles, one by one; plus the invariant that holds at any size,
-    momentum conservation sum_i F_i = 0 (interlace 0)."""
-    pos, c = gen.make_config_positions("headline")
-    n = pos.shape[0]
-    f = gpu_force(pm, params_of(pm, c, n), pos)
-    kw = oracle_kw(c)
-    kw.pop("interlace")
-    d = po.density_contrast(po.scatter(pos, c["m"], c["box"], kw["worder"]), n)
-    g = po.poisson_force(d, box=c["box"], **kw)
-    del d
-    idx = np.sort(np.random.default_rng(4242).choice(n, size=200_000, replace=False))
-    ref = np.stack([po.gather(g[a], pos[idx], c["box"], kw["worder"]) for a in range(3)], axis=1)
-    err = rel_l2(f[idx], ref)
-    record_error("force/headline/n_p=512/sampled=200000", err, FORCE_TOL)
-    assert err <= FORCE_TOL
-    fsum = np.abs(f.astype(np.float64).sum(axis=0)).max()
-    assert fsum <= 1e-6 * np.abs(f.astype(np.float64)).sum()

@@ -14,7 +14,7 @@ torch = pytest.importorskip("torch")
 from oracle import pm_oracle as po
 from pm_inputs import generators as gen
 
-from conftest import record_error
+from parity_util import check, record_error, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -30,12 +30,6 @@ def pm():
     import paper_2510_05206_b200 as pm_
 
     return pm_
-
-
-def rel_l2(a, b):
-    a = np.asarray(a, dtype=np.float64)
-    b = np.asarray(b, dtype=np.float64)
-    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
 
 
 def dev(x):
@@ -65,7 +59,7 @@ def test_assign_parity(pm, worder, shift_cells):
     mesh = torch.zeros(M, M, M, device="cuda")
     pm.pm_assign(ctx, dev(pos), None, mesh, shift=shift)
     ref = po.scatter(pos, M, BOX, worder, shift=shift)
-    assert rel_l2(mesh.cpu().numpy(), ref) <= 1e-6
+    check("mesh", mesh, ref, 1e-6)
     # exact mass conservation (partition of unity), to fp32 accumulation
     assert abs(float(mesh.double().sum()) - pos.shape[0]) <= 1e-6 * pos.shape[0]
     # weighted, accumulating onto a pre-existing mesh
@@ -74,7 +68,7 @@ def test_assign_parity(pm, worder, shift_cells):
     mesh2 = dev(pre)
     pm.pm_assign(ctx, dev(pos), dev(w), mesh2, shift=shift)
     ref2 = po.scatter(pos, M, BOX, worder, weights=w, shift=shift, mesh=pre.astype(np.float64))
-    assert rel_l2(mesh2.cpu().numpy(), ref2) <= 1e-6
+    check("mesh2", mesh2, ref2, 1e-6)
     pm.pm_destroy(ctx)
 
 
@@ -89,7 +83,7 @@ def test_interp_parity(pm, worder, shift_cells, ncomp):
     out = torch.empty(pos.shape[0], ncomp, device="cuda")
     pm.pm_interp(ctx, [dev(meshes[a]) for a in range(ncomp)], dev(pos), out, shift=shift)
     ref = np.stack([po.gather(meshes[a], pos, BOX, worder, shift=shift) for a in range(ncomp)], axis=1)
-    assert rel_l2(out.cpu().numpy(), ref) <= 1e-6
+    check("out", out, ref, 1e-6)
     pm.pm_destroy(ctx)
 
 
@@ -107,8 +101,8 @@ def test_assign_vjp_parity(pm, worder, shifted):
     pm.pm_assign_vjp(ctx, dev(pos), dev(w), dev(cot), pos_cot=pos_cot, w_cot=w_cot, shift=shift)
     ref_w = po.gather(cot, pos, BOX, worder, shift=shift)
     ref_p = np.stack([w * po.gather(cot, pos, BOX, worder, shift=shift, deriv_axis=b) for b in range(3)], axis=1)
-    assert rel_l2(w_cot.cpu().numpy(), ref_w) <= 1e-6
-    assert rel_l2(pos_cot.cpu().numpy(), ref_p) <= 2e-6
+    check("w_cot", w_cot, ref_w, 1e-6)
+    check("pos_cot", pos_cot, ref_p, 2e-6)
     pm.pm_destroy(ctx)
 
 
@@ -128,12 +122,12 @@ def test_interp_vjp_parity(pm, worder, ncomp):
         # random-sign weights in a dense clump: the node sums cancel, while the fixed-point quantum is 2^-30 of the
         # work item's bound sum|w| * Wmax^3 ("Parity bars"); with items of up to 4096 particles that is
         # the accuracy of an fp32 accumulation in the same order, not better
-        assert rel_l2(mesh_cot[a].cpu().numpy(), ref) <= 5e-6
+        check("mesh_cot[a]", mesh_cot[a], ref, 5e-6)
     ref_p = np.zeros((n, 3))
     for a in range(ncomp):
         for b in range(3):
             ref_p[:, b] += cot[:, a] * po.gather(meshes[a], pos, BOX, worder, deriv_axis=b)
-    assert rel_l2(pos_cot.cpu().numpy(), ref_p) <= 2e-6
+    check("pos_cot", pos_cot, ref_p, 2e-6)
     pm.pm_destroy(ctx)
 
 
@@ -167,13 +161,13 @@ def test_poisson_force_parity(pm, grad_order, lap_order, deconv_pow, worder):
     pm.pm_poisson_force(ctx, dev(delta), g)
     ref = po.poisson_force(delta, box, worder, grad_order, lap_order, deconv_pow, coeff=1.7)
     for a in range(3):
-        assert rel_l2(g[a].cpu().numpy(), ref[a]) <= 2e-6
+        check("g[a]", g[a], ref[a], 2e-6)
     # transpose
     cot = gen.random_mesh(m, 13, 3)
     dc = torch.empty(m, m, m, device="cuda")
     pm.pm_poisson_force_vjp(ctx, [dev(cot[a]) for a in range(3)], dc)
     refv = po.poisson_force_vjp([cot[a] for a in range(3)], box, worder, grad_order, lap_order, deconv_pow, coeff=1.7)
-    assert rel_l2(dc.cpu().numpy(), refv) <= 2e-6
+    check("dc", dc, refv, 2e-6)
     pm.pm_destroy(ctx)
 
 
@@ -185,14 +179,14 @@ def test_poisson_force_interlaced_parity(pm):
     pm.pm_poisson_force(ctx, dev(d[0]), g, delta_mesh2=dev(d[1]))
     ref = po.poisson_force(d[0], box, 3, 4, 0, 2, delta_mesh2=d[1])
     for a in range(3):
-        assert rel_l2(g[a].cpu().numpy(), ref[a]) <= 2e-6
+        check("g[a]", g[a], ref[a], 2e-6)
     cot = gen.random_mesh(m, 15, 3)
     c1 = torch.empty(m, m, m, device="cuda")
     c2 = torch.empty(m, m, m, device="cuda")
     pm.pm_poisson_force_vjp(ctx, [dev(cot[a]) for a in range(3)], c1, delta_cot2=c2)
     r1, r2 = po.poisson_force_vjp([cot[a] for a in range(3)], box, 3, 4, 0, 2, interlace=True)
-    assert rel_l2(c1.cpu().numpy(), r1) <= 2e-6
-    assert rel_l2(c2.cpu().numpy(), r2) <= 2e-6
+    check("c1", c1, r1, 2e-6)
+    check("c2", c2, r2, 2e-6)
     pm.pm_destroy(ctx)
 
 
@@ -203,18 +197,18 @@ def test_edge_cases(pm):
     p1 = np.array([[7.9, 0.05, 3.5]], dtype=np.float32)
     mesh = torch.zeros(8, 8, 8, device="cuda")
     pm.pm_assign(ctx, dev(p1), None, mesh)
-    assert rel_l2(mesh.cpu().numpy(), po.scatter(p1, 8, 8.0, 4)) <= 1e-6
+    check("one_particle", mesh, po.scatter(p1, 8, 8.0, 4), 1e-6)
     # 20000 particles inside one cell of an 8^3 mesh whose kernel support wraps around the box
     rng = np.random.default_rng(3)
     pc = (rng.random((20000, 3)) * 0.9 + np.array([7.05, 0.05, 7.05])).astype(np.float32) % np.float32(8.0)
     mesh.zero_()
     pm.pm_assign(ctx, dev(pc), None, mesh)
-    assert rel_l2(mesh.cpu().numpy(), po.scatter(pc, 8, 8.0, 4)) <= 1e-6
+    check("one_cell", mesh, po.scatter(pc, 8, 8.0, 4), 1e-6)
     f = gen.random_mesh(8, 4, 3)
     out = torch.empty(20000, 3, device="cuda")
     pm.pm_interp(ctx, [dev(f[a]) for a in range(3)], dev(pc), out)
     ref = np.stack([po.gather(f[a], pc, 8.0, 4) for a in range(3)], axis=1)
-    assert rel_l2(out.cpu().numpy(), ref) <= 1e-6
+    check("out", out, ref, 1e-6)
     pm.pm_destroy(ctx)
 
 
@@ -234,32 +228,31 @@ def test_bucket_overflow_of_single_pass_binning(pm):
         mesh = torch.zeros(m, m, m, device="cuda")
         pm.pm_assign(ctx, dev(pos), None, mesh)
         ref = po.scatter(pos, m, box, worder)
-        assert rel_l2(mesh.cpu().numpy(), ref) <= 1e-6
+        check("mesh", mesh, ref, 1e-6)
         assert abs(float(mesh.sum().cpu()) - n) <= 1e-4 * n
         f = gen.random_mesh(m, 5, 3)
         out = torch.empty(n, 3, device="cuda")
         pm.pm_interp(ctx, [dev(f[a]) for a in range(3)], dev(pos), out)
         refg = np.stack([po.gather(f[a], pos, box, worder) for a in range(3)], axis=1)
-        assert rel_l2(out.cpu().numpy(), refg) <= 1e-6
+        check("out", out, refg, 1e-6)
         pm.pm_destroy(ctx)
 
 
-def test_two_pass_binning_path_matches(pm, monkeypatch):
+def test_two_pass_binning_path_matches(pm):
     """The two-pass (histogram + permute) binning, kept for N too large for 32-bit bucket indices and selectable
-    with PMF_BIN_TWOPASS=1, must give the same assignment and forces as the default single-pass path."""
+    with PM_FLAG_BIN_TWOPASS, must give the same assignment and forces as the default single-pass path."""
     pos, c = gen.make_config_positions("cfg4", n_p=32)
     n = pos.shape[0]
     f = gen.random_mesh(c["m"], 6, 3)
     ref = po.scatter(pos, c["m"], c["box"], 2)
     outs = []
-    for two_pass in ("0", "1"):
-        monkeypatch.setenv("PMF_BIN_TWOPASS", two_pass)
-        ctx = pm.pm_create(pm.PMParams(m=c["m"], box=c["box"], max_particles=n, worder=2))
+    for flags in (0, pm.FLAG_BIN_TWOPASS):
+        ctx = pm.pm_create(pm.PMParams(m=c["m"], box=c["box"], max_particles=n, worder=2, flags=flags))
         mesh = torch.zeros(c["m"], c["m"], c["m"], device="cuda")
         pm.pm_assign(ctx, dev(pos), None, mesh)
         out = torch.empty(n, 3, device="cuda")
         pm.pm_interp(ctx, [dev(f[a]) for a in range(3)], dev(pos), out)
-        assert rel_l2(mesh.cpu().numpy(), ref) <= 1e-6
+        check("mesh", mesh, ref, 1e-6)
         outs.append(out.cpu().numpy())
         pm.pm_destroy(ctx)
     # the gather of one particle does not depend on how the records were sorted
@@ -276,3 +269,41 @@ def test_errors_are_reported(pm):
     with pytest.raises(pm.PMError):
         pm.nufft_spread(ctx, pos[:4], None, torch.zeros(16, 16, 16, device="cuda"))  # PM ctx
     pm.pm_destroy(ctx)
+
+
+def test_pm_bin_pinned_records_are_reused(pm):
+    """pm_bin pins the sorted records: pm_assign, pm_interp, pm_interp_vjp and pm_assign_vjp given the same
+    (pos, N) reuse them (include/pmforce.h); results must equal the calls that bin internally, and a call with
+    other positions must drop the pin and bin again."""
+    pos = mixed_positions(20000, BOX, 91)
+    n = pos.shape[0]
+    d_pos = dev(pos)
+    meshes = gen.random_mesh(M, 92, 3)
+    d_m = [dev(meshes[a]) for a in range(3)]
+    cot = gen.gaussian_cotangent(n, 93, 3)
+    for worder in (2, 3):
+        ctx = pm.pm_create(pm.PMParams(m=M, box=BOX, max_particles=n, worder=worder))
+        pm.pm_bin(ctx, d_pos)
+        mesh = torch.zeros(M, M, M, device="cuda")
+        pm.pm_assign(ctx, d_pos, None, mesh)
+        check("pinned/assign", mesh, po.scatter(pos, M, BOX, worder), 1e-6)
+        out = torch.empty(n, 3, device="cuda")
+        pm.pm_interp(ctx, d_m, d_pos, out)
+        ref = np.stack([po.gather(meshes[a], pos, BOX, worder) for a in range(3)], axis=1)
+        check("pinned/interp", out, ref, 1e-6)
+        pc = torch.empty(n, 3, device="cuda")
+        mc = [torch.zeros(M, M, M, device="cuda") for _ in range(3)]
+        pm.pm_interp_vjp(ctx, d_m, d_pos, dev(cot), mesh_cot=mc, pos_cot=pc)
+        refp = np.zeros((n, 3))
+        for a in range(3):
+            check(f"pinned/mesh_cot{a}", mc[a], po.scatter(pos, M, BOX, worder, weights=cot[:, a]), 5e-6)
+            for b in range(3):
+                refp[:, b] += cot[:, a] * po.gather(meshes[a], pos, BOX, worder, deriv_axis=b)
+        check("pinned/pos_cot", pc, refp, 2e-6)
+        # other positions at another address: the pin is dropped, the records are rebuilt
+        pos2 = mixed_positions(20000, BOX, 94)
+        out2 = torch.empty(n, 3, device="cuda")
+        pm.pm_interp(ctx, d_m, dev(pos2), out2)
+        ref2 = np.stack([po.gather(meshes[a], pos2, BOX, worder) for a in range(3)], axis=1)
+        check("repinned/interp", out2, ref2, 1e-6)
+        pm.pm_destroy(ctx)

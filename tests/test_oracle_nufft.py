@@ -144,3 +144,14 @@ def test_kernel_gradient_force_vs_bruteforce(sigma, width, tol):
     k[np.abs(np.fft.fftfreq(mf, 1.0 / mf)) >= 0.5 * m] = 0.0
     spec = np.fft.ifft(-1j * k[:, None, None] * np.fft.fft(phi, axis=0), axis=0).real
     assert np.abs(spec - gx).max() < 1e-10 * np.abs(gx).max()
+
+
+def test_kspace_multiplier_at_matches_the_arrays():
+    mf, m, box, n, w, beta = 16, 8, 10.0, 300, 7, 16.1
+    M = no._kspace_multiplier(mf, m, box, n, w, beta, 1.4)
+    rng = np.random.default_rng(80)
+    idx = (rng.integers(0, mf, 300), rng.integers(0, mf, 300), rng.integers(0, mf // 2 + 1, 300))
+    idx[0][:2] = idx[1][:2] = idx[2][:2] = 0
+    Ma = no.kspace_multiplier_at(idx, mf, m, box, n, w, beta, 1.4)
+    for a in range(3):
+        assert np.allclose(M[a][idx], Ma[a], rtol=1e-14, atol=0)

@@ -275,3 +275,17 @@ def test_real_space_gradient_equals_fourier_symbol(order, interlaced):
     err = np.abs(po.fd_gradient_real(f, box, order, 0) - exact).max() / (2 * np.pi / box)
     assert err < {2: 0.05, 4: 4e-3, 6: 4e-4}[order]
     assert np.abs(po.fd_gradient_real(f, box, order, 1)).max() < 1e-14
+
+
+def test_force_symbol_at_matches_the_symbol_arrays():
+    m, box = 12, 30.0
+    rng = np.random.default_rng(70)
+    idx = tuple(rng.integers(0, m, 200) for _ in range(2)) + (rng.integers(0, m // 2 + 1, 200),)
+    idx[0][:3] = idx[1][:3] = idx[2][:3] = 0          # the n = 0 mode
+    idx[0][3:6] = m // 2                              # Nyquist planes
+    idx[2][6:9] = m // 2
+    for go, lo, dp, wo in ((0, 0, 2, 2), (4, 0, 2, 3), (6, 6, 1, 4), (2, 2, 0, 2)):
+        S = po.force_symbols(m, box, wo, go, lo, dp, 1.7)
+        Sa = po.force_symbol_at(idx, m, box, wo, go, lo, dp, 1.7)
+        for a in range(3):
+            assert np.array_equal(S[a][idx], Sa[a])

@@ -132,6 +132,21 @@ int pm_interp_vjp(pm_ctx* ctx, const float* const mesh[], int ncomp, const float
                   const double* shift, const float* out_cot, float* const mesh_cot[], float* pos_cot,
                   void* stream);
 
+/* ---- NEXT-2: forward-mode rules, Eq. C.13, rule table :956-960 (method 0) ---------- */
+/* Tangent of pm_assign, Eq. C.13a:
+ *   mesh_tan[j] += sum_i [ w_tan[i] W_j(X_i) + w_i pos_tan[i,:] . dW_j(X_i)/dX_i ]     (-grad W_j = dW_j/dX_i, :860)
+ * ACCUMULATES onto mesh_tan, which the caller initialises with the tangent of the input mesh (Eq. C.4) or zero.
+ * w: [N] or NULL (ones); pos_tan: [N,3] or NULL (0); w_tan: [N] or NULL (0). */
+int pm_assign_jvp(pm_ctx* ctx, const float* pos, const float* w, int64_t N, const double* shift,
+                  const float* pos_tan, const float* w_tan, float* mesh_tan, void* stream);
+/* Tangent of pm_interp, Eq. C.13b (ncomp = 1 or 3):
+ *   out_tan[i,a] = sum_j [ mesh_tan[a][j] W_j(X_i) + mesh[a][j] pos_tan[i,:] . dW_j(X_i)/dX_i ]
+ * mesh_tan: host array of ncomp device pointers or NULL (0); pos_tan: [N,3] or NULL (0); out_tan: [N,ncomp],
+ * overwritten. */
+int pm_interp_jvp(pm_ctx* ctx, const float* const mesh[], int ncomp, const float* pos, int64_t N,
+                  const double* shift, const float* pos_tan, const float* const mesh_tan[], float* out_tan,
+                  void* stream);
+
 /* ---- a6-a8, a12: NUFFT path (method = 1), exponential-of-semicircle kernel ------- */
 /* fine[j] += sum_i c_i prod_a phi(2 (j_a - u_a)/w), u = X / (box/m_f); phi(z) = exp(beta (sqrt(1-z^2)-1)).
  * ACCUMULATES.  c: [N] or NULL (ones). */
@@ -155,10 +170,44 @@ int nufft_interp_vjp(pm_ctx* ctx, const float* const fine[], int ncomp, const fl
  * density contrast delta = (m^3/N) rho - 1 of Eq. 2.3 PAPER.md:92 is folded into the k-space kernel) or
  * a0, a6-a8 (method 1).  force: [N,3], overwritten. */
 int pm_force(pm_ctx* ctx, const float* pos, int64_t N, float* force, void* stream);
-/* pos_cot = force_cot^T dA/dX (a9-a11; App. C).  Recomputes the forward meshes.
- * force_cot: [N,3]; pos_cot: [N,3], overwritten. */
+/* pos_cot = force_cot^T dA/dX (a9-a11; App. C).  force_cot: [N,3]; pos_cot: [N,3],
+ * overwritten.  The forward meshes are recomputed, unless the records are pinned (pm_bin) and the last pm_force
+ * on this ctx ran on the pinned (pos, N): then its force meshes are reused (interlace 0 or 1). */
 int pm_force_vjp(pm_ctx* ctx, const float* pos, int64_t N, const float* force_cot, float* pos_cot,
                  void* stream);
+/* ---- NEXT-1: drift-kick-drift step (Eq. 2.14a-c) and its backward-in-time adjoint ----- */
+/* One step, in place:  X <- X + tau1 V;  V <- alpha V + beta A(X);  X <- X + tau2 V   (A = pm_force of this ctx).
+ * pos, vel: [N,3] device arrays, both overwritten.  Positions are kept in [0, box): every drift wraps, in fp32
+ * arithmetic that is specified operation by operation (reading R18) so that a CPU reference evaluates
+ * the force at bitwise the same positions.  The kick and the second drift run in the epilogue of the gather; no
+ * force array is written.  alpha, beta, tau1, tau2 are plain scalars (Eq. 2.15-2.17 are the caller's business).
+ * Drops any pm_bin pin (the positions change).  PM_ESTATE for a ctx with PM_FLAG_KERNEL_GRAD. */
+int pm_dkd_step(pm_ctx* ctx, float* pos, float* vel, int64_t N, double tau1, double tau2, double alpha,
+                double beta, void* stream);
+/* The backward-in-time step of Table 3, rows in the table's order, in place:
+ *   in : (X^n, V^n, X*^n, V*^n)        out: (X^{n-1}, V^{n-1}, X*^{n-1}, V*^{n-1})
+ * with the same (tau1, tau2, alpha, beta) the forward step n-1 -> n used.  The acceleration A(X^{n-1/2}) and
+ * its VJP with V*^{n-1/2} share ONE set of forward meshes.  scalar_adj: device pointer to 4
+ * doubles or NULL; receives the adjoints of the temporal coefficients of this step {tau1*, tau2*, alpha*,
+ * beta*} (overwritten; alpha* = V*^{n-1/2} . V^{n-1}: DESIGN.md reading R19). */
+int pm_dkd_step_adjoint(pm_ctx* ctx, float* pos, float* vel, float* pos_adj, float* vel_adj, int64_t N,
+                        double tau1, double tau2, double alpha, double beta, double* scalar_adj, void* stream);
+
+/* ---- NEXT-4: analysis ------------------------------------------------------------------------------- */
+/* Shell-averaged (cross-)power spectrum of the density of `pos` (x `pos2`; NULL = auto spectrum).
+ * The density is assigned with the ctx's worder and, if interlace = 1, combined from two interlaced grids;
+ * deconvolve != 0 divides by ONE power of the assignment window (reading R20).  Bin b (0 <= b < nbins,
+ * nbins <= m) holds the modes of the full Fourier cube with b + 1/2 <= |n| < b + 3/2, k = 2 pi n / box.
+ * Outputs: device arrays of nbins doubles: mean |k| of the bin, P = box^3 <Re(dA conj dB)> / m^6 (no shot-noise
+ * subtraction), number of modes; empty bins give 0.  method 0 only. */
+int pm_power_spectrum(pm_ctx* ctx, const float* pos, int64_t N, const float* pos2, int64_t N2, int deconvolve,
+                      int nbins, double* k_mean, double* power, double* n_modes, void* stream);
+/* Sheet-based resampling, trilinear variant (Table 5 n_resample :411; reading R21).
+ * pos: [n_p^3, 3] in Lagrangian (C) order (particle (i,j,k) started at (i,j,k) box/n_p); pos_out:
+ * [(r n_p)^3, 3], the refined sheet X' = q' + trilinear interpolation of the displacement, wrapped into
+ * [0, box); feed it to pm_assign with weights r^-3.  Any ctx with the right box serves (m is not used). */
+int pm_sheet_resample(pm_ctx* ctx, const float* pos, int32_t n_p, int32_t r, float* pos_out, void* stream);
+
 /* Same as pm_force with HOST buffers: copies pos_host to the device, runs pm_force, copies the forces
  * back and synchronises.  Pinned host memory gives asynchronous copies; pageable memory also works. */
 int pm_force_host(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream);
@@ -175,7 +224,9 @@ int pm_set_profiling(pm_ctx* ctx, int enable);
 #define PM_STAGE_VJP_SCATTER 6
 #define PM_STAGE_VJP_KSPACE 7 /* 3 R2C + transposed kernel + C2R */
 #define PM_STAGE_VJP_GATHER 8
-#define PM_NUM_STAGES 9
+#define PM_STAGE_GRADIENT 9 /* real-space stencil of PM_FLAG_GRAD_REAL */
+#define PM_STAGE_STEP 10    /* drift / adjoint-drift kernels of pm_dkd_step(_adjoint) */
+#define PM_NUM_STAGES 11
 /* Synchronises on the last profiled call and writes the duration in ms of each stage (0 if it did not
  * run) to ms_host[0..n-1], n <= PM_NUM_STAGES.  launches_host (or NULL) receives how many kernels of
  * this library (cuFFT's excluded) that call launched. */

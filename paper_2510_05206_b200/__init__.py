@@ -28,6 +28,12 @@ from .api import (  # noqa: F401
     pm_force,
     pm_force_vjp,
     pm_force_host,
+    pm_assign_jvp,
+    pm_interp_jvp,
+    pm_dkd_step,
+    pm_dkd_step_adjoint,
+    pm_power_spectrum,
+    pm_sheet_resample,
     pm_set_profiling,
     pm_get_stage_ms,
     STAGE_NAMES,

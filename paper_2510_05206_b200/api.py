@@ -14,10 +14,12 @@ EXPORTED_SYMBOLS = (
     "pm_nufft_beta", "pm_bin", "pm_assign", "pm_assign_vjp", "pm_poisson_force", "pm_poisson_force_vjp",
     "pm_interp", "pm_interp_vjp", "nufft_spread", "nufft_spread_vjp", "nufft_poisson_force",
     "nufft_poisson_force_vjp", "nufft_interp", "nufft_interp_vjp", "pm_force", "pm_force_vjp", "pm_force_host",
-    "pm_set_profiling", "pm_get_stage_ms",
+    "pm_set_profiling", "pm_get_stage_ms", "pm_assign_jvp", "pm_interp_jvp", "pm_dkd_step", "pm_dkd_step_adjoint",
+    "pm_power_spectrum", "pm_sheet_resample",
 )
 
-STAGE_NAMES = ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "interp", "vjp_scatter", "vjp_kspace", "vjp_gather")
+STAGE_NAMES = ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "interp", "vjp_scatter", "vjp_kspace", "vjp_gather",
+               "gradient", "step")
 
 
 FLAG_BIN_TWOPASS, FLAG_NO_XFUSE, FLAG_GRAD_REAL, FLAG_KERNEL_GRAD = 1, 2, 4, 8  # pm_params.flags
@@ -107,6 +109,13 @@ def load_library(build_if_missing: bool = False):
         "pm_force": (C.c_int, [vp, vp, i64, vp, vp]),
         "pm_force_vjp": (C.c_int, [vp, vp, i64, vp, vp, vp]),
         "pm_force_host": (C.c_int, [vp, vp, i64, vp, vp]),
+        "pm_assign_jvp": (C.c_int, [vp, vp, vp, i64, f64p, vp, vp, vp, vp]),
+        "pm_interp_jvp": (C.c_int, [vp, C.POINTER(vp), C.c_int, vp, i64, f64p, vp, C.POINTER(vp), vp, vp]),
+        "pm_dkd_step": (C.c_int, [vp, vp, vp, i64, C.c_double, C.c_double, C.c_double, C.c_double, vp]),
+        "pm_dkd_step_adjoint": (C.c_int, [vp, vp, vp, vp, vp, i64, C.c_double, C.c_double, C.c_double, C.c_double,
+                                          vp, vp]),
+        "pm_power_spectrum": (C.c_int, [vp, vp, i64, vp, i64, C.c_int, C.c_int, vp, vp, vp, vp]),
+        "pm_sheet_resample": (C.c_int, [vp, vp, C.c_int32, C.c_int32, vp, vp]),
         "pm_set_profiling": (C.c_int, [vp, C.c_int]),
         "pm_get_stage_ms": (C.c_int, [vp, C.POINTER(C.c_float), C.c_int, C.POINTER(i64)]),
     }
@@ -310,6 +319,64 @@ def pm_force_vjp(ctx, pos, force_cot, pos_cot):
     n = _n(pos)
     ctx.check(load_library().pm_force_vjp(ctx.handle, _dev(pos, "pos"), n, _dev(force_cot, "force_cot", 3 * n),
                                           _dev(pos_cot, "pos_cot", 3 * n), _stream()), "pm_force_vjp")
+
+
+def pm_assign_jvp(ctx, pos, w, mesh_tan, pos_tan=None, w_tan=None, shift=None):
+    n = _n(pos)
+    ctx.check(load_library().pm_assign_jvp(ctx.handle, _dev(pos, "pos"), _dev(w, "w", n), n, _shift(shift),
+                                           _dev(pos_tan, "pos_tan", 3 * n), _dev(w_tan, "w_tan", n),
+                                           _dev(mesh_tan, "mesh_tan", ctx.G), _stream()), "pm_assign_jvp")
+
+
+def pm_interp_jvp(ctx, mesh, pos, out_tan, pos_tan=None, mesh_tan=None, shift=None):
+    n, ncomp = _n(pos), len(mesh)
+    ctx.check(load_library().pm_interp_jvp(ctx.handle, _ptr_array(mesh, "mesh", ctx.G), ncomp, _dev(pos, "pos"), n,
+                                           _shift(shift), _dev(pos_tan, "pos_tan", 3 * n),
+                                           _ptr_array(mesh_tan, "mesh_tan", ctx.G),
+                                           _dev(out_tan, "out_tan", n * ncomp), _stream()), "pm_interp_jvp")
+
+
+def _dev64(t, name: str, numel: int):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float64 CUDA tensor")
+    if t.numel() != numel:
+        raise ValueError(f"{name} has {t.numel()} elements, expected {numel}")
+    return t.data_ptr()
+
+
+def pm_dkd_step(ctx, pos, vel, tau1, tau2, alpha, beta):
+    """In place: pos, vel [N,3] (Eq. 2.14a-c)."""
+    n = _n(pos)
+    ctx.check(load_library().pm_dkd_step(ctx.handle, _dev(pos, "pos"), _dev(vel, "vel", 3 * n), n, float(tau1),
+                                         float(tau2), float(alpha), float(beta), _stream()), "pm_dkd_step")
+
+
+def pm_dkd_step_adjoint(ctx, pos, vel, pos_adj, vel_adj, tau1, tau2, alpha, beta, scalar_adj=None):
+    """In place: pos, vel, pos_adj, vel_adj [N,3] (Table 3); scalar_adj: float64 CUDA tensor [4] or None."""
+    n = _n(pos)
+    ctx.check(load_library().pm_dkd_step_adjoint(ctx.handle, _dev(pos, "pos"), _dev(vel, "vel", 3 * n),
+                                                 _dev(pos_adj, "pos_adj", 3 * n), _dev(vel_adj, "vel_adj", 3 * n), n,
+                                                 float(tau1), float(tau2), float(alpha), float(beta),
+                                                 _dev64(scalar_adj, "scalar_adj", 4), _stream()),
+              "pm_dkd_step_adjoint")
+
+
+def pm_power_spectrum(ctx, pos, k_mean, power, n_modes, pos2=None, deconvolve=True):
+    """k_mean, power, n_modes: float64 CUDA tensors [nbins]."""
+    nbins = k_mean.numel()
+    ctx.check(load_library().pm_power_spectrum(ctx.handle, _dev(pos, "pos"), _n(pos), _dev(pos2, "pos2"),
+                                               _n(pos2) if pos2 is not None else 0, int(bool(deconvolve)), nbins,
+                                               _dev64(k_mean, "k_mean", nbins), _dev64(power, "power", nbins),
+                                               _dev64(n_modes, "n_modes", nbins), _stream()), "pm_power_spectrum")
+
+
+def pm_sheet_resample(ctx, pos, n_p, r, pos_out):
+    if _n(pos) != n_p ** 3 or _n(pos_out) != (n_p * r) ** 3:
+        raise ValueError("pos must hold n_p^3 and pos_out (r n_p)^3 particles")
+    ctx.check(load_library().pm_sheet_resample(ctx.handle, _dev(pos, "pos"), int(n_p), int(r),
+                                               _dev(pos_out, "pos_out"), _stream()), "pm_sheet_resample")
 
 
 def pm_force_host(ctx, pos_host, force_host):

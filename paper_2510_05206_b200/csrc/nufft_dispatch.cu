@@ -36,9 +36,10 @@ int launch_es_scatter(Ctx* c, int ncomp, const float* wsrc, int wstride, float* 
 
 int launch_es_gather(Ctx* c, const GatherArgs& a, cudaStream_t st) {
   if (c->bin_n == 0) return PM_OK;
+  if (a.mode == GATHER_JVP) return fail(c, PM_ESTATE, "forward-mode gathers are built for the PM kernels only");
   switch (c->nufft_w) {
 #define CASE(W) \
-  case W: return a.grad ? es_gather_grad_w<W>(c, a, st) : es_gather_values_w<W>(c, a, st);
+  case W: return a.mode == GATHER_GRAD ? es_gather_grad_w<W>(c, a, st) : es_gather_values_w<W>(c, a, st);
     ES_WIDTHS(CASE)
 #undef CASE
   }

@@ -31,11 +31,12 @@ int es_scatter_w<ES_W>(Ctx* c, int ncomp, const float* wsrc, int wstride, float*
   const typename T::Params tp = es_params<T>(c);
   const int roll[3] = {0, 0, 0};
   if (!wsrc) {
-    for (int a = 0; a < ncomp; ++a) PM_TRY((run_scatter<T, 1, false>(c, tp, roll, nullptr, 0, mesh + a, st)));
+    for (int a = 0; a < ncomp; ++a) PM_TRY((run_scatter<T, 1, W_UNIT>(c, tp, roll, weights_src(nullptr, 0), mesh + a, st)));
     return PM_OK;
   }
-  if (ncomp == 3) return run_scatter<T, 3, true>(c, tp, roll, wsrc, wstride, mesh, st);
-  for (int a = 0; a < ncomp; ++a) PM_TRY((run_scatter<T, 1, true>(c, tp, roll, wsrc + a, wstride, mesh + a, st)));
+  if (ncomp == 3) return run_scatter<T, 3, W_WEIGHTED>(c, tp, roll, weights_src(wsrc, wstride), mesh, st);
+  for (int a = 0; a < ncomp; ++a)
+    PM_TRY((run_scatter<T, 1, W_WEIGHTED>(c, tp, roll, weights_src(wsrc + a, wstride), mesh + a, st)));
   return PM_OK;
 }
 
@@ -45,8 +46,7 @@ static int go(Ctx* c, const GatherArgs& a, cudaStream_t st) {
   constexpr size_t smem = sizeof(float) * (size_t)NCOMP * Geo<T>::COMP + 128;
   if (smem > 200 * 1024) return fail(c, PM_EINVAL, "ES gather: %d meshes of width %d do not fit in shared memory", NCOMP, T::P);
   const int roll[3] = {0, 0, 0};
-  return run_gather<T, NCOMP, GRAD>(c, es_params<T>(c), roll, a.mesh, a.cot, a.cstride, a.ncot, a.const_coef, a.wmul,
-                                    a.alpha, a.accumulate, a.out, st);
+  return run_gather<T, NCOMP, GRAD ? G_GRAD : G_VALUES>(c, es_params<T>(c), roll, a, st);
 }
 
 #if ES_PART == 1

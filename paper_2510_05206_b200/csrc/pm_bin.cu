@@ -475,6 +475,7 @@ int ensure_bins(Ctx* c, const float* pos, int64_t N, cudaStream_t st, bool pin) 
   if (N < 0 || N > c->cap) return fail(c, PM_EINVAL, "N = %lld outside [0, max_particles = %lld]", (long long)N, (long long)c->cap);
   if (!pin && c->bin_valid && c->bin_pinned && c->bin_pos == pos && c->bin_n == N) return PM_OK;
   c->bin_valid = false;
+  c->g_valid = false;  // force meshes of other records
   BinGeom g;
   g.m = c->mg;
   g.ntx = c->ntx;
@@ -566,5 +567,7 @@ int bin_occupancy(int pass) {
 
 extern "C" int pm_bin(pm_ctx* ctx, const float* pos, int64_t N, void* stream) {
   if (!ctx) return PM_EINVAL;
+  const int rc = pmf::enter_device(pmf::C(ctx));
+  if (rc != PM_OK) return rc;
   return pmf::ensure_bins(pmf::C(ctx), pos, N, (cudaStream_t)stream, true);
 }

@@ -288,6 +288,15 @@ static int build(Ctx* c) {
   PM_TRY(upload(c, &c->tab_win, w));
   PM_TRY(upload(c, &c->tab_cos, pc));
   PM_TRY(upload(c, &c->tab_sin, ps));
+  {  // W~(n) to the first power (pm_power_spectrum)
+    std::vector<double> w1(mg, 1.0);
+    if (p.method == 0)
+      for (int i = 0; i < mg; ++i) {
+        const int n = (i < (mg + 1) / 2) ? i : i - mg;
+        w1[i] = pow(sinc_pi((double)n / (double)mg), (double)p.worder);
+      }
+    PM_TRY(upload(c, &c->tab_win1, w1));
+  }
 
   // binning workspace
   c->cap = p.max_particles;
@@ -370,7 +379,8 @@ static void teardown(Ctx* c) {
     cufftDestroy(c->plan2_r2c);
     cufftDestroy(c->plan2_c2r);
   }
-  void* ptrs[] = {c->tab_grad, c->tab_lap, c->tab_win, c->tab_cos, c->tab_sin, c->rec, c->tile_cnt,
+  void* ptrs[] = {c->tab_grad, c->tab_lap, c->tab_win, c->tab_cos, c->tab_sin, c->tab_win1, c->phi, c->step_dots,
+                  c->ps_acc, c->rec, c->tile_cnt,
                   c->tile_off, c->item_off, c->scan_tmp, c->items, c->nitems, c->sched, c->fft_work, c->rho[0],
                   c->rho[1], c->dhat[0], c->dhat[1], c->ghat[0], c->ghat[1], c->ghat[2], c->g[0],
                   c->g[1], c->g[2], c->gbar[0], c->gbar[1], c->gbar[2], c->xtw, c->xsym, c->xph, c->ov_count, c->ov_rec, c->ov_tile, c->ov_cur,
@@ -381,6 +391,12 @@ static void teardown(Ctx* c) {
   if (c->ev_ok)
     for (int i = 0; i < 2 * PM_NUM_STAGES; ++i) cudaEventDestroy(c->ev[i]);
   free(c);
+}
+
+int ensure_phi(Ctx* c) {
+  if (c->phi) return PM_OK;
+  PM_CUDA(c, cudaMalloc((void**)&c->phi, sizeof(float) * (size_t)c->G));
+  return PM_OK;
 }
 
 void stage_begin(Ctx* c, int stage, cudaStream_t st) {

@@ -58,6 +58,19 @@ __host__ __device__ __forceinline__ uint32_t tile_id(int tx, int ty, int tz, int
 
 enum { MAX_W = 16 };
 
+// Periodic wrap into [0, L) in fp32, operation by operation as DESIGN.md reading R18 specifies.
+__device__ __forceinline__ float wrap_box_fp32(float x, float L) {
+  float y = __fsub_rn(x, __fmul_rn(L, floorf(__fdiv_rn(x, L))));
+  if (y < 0.0f) y = __fadd_rn(y, L);
+  if (y >= L) y = __fsub_rn(y, L);
+  if (y >= L || y < 0.0f) y = 0.0f;
+  return y;
+}
+__device__ __forceinline__ float drift_fp32(float x, float v, float tau, float L) {
+  return wrap_box_fp32(__fadd_rn(x, __fmul_rn(tau, v)), L);
+}
+
+
 struct Ctx;
 
 // ---- error helpers ------------------------------------------------------------------------------
@@ -109,6 +122,7 @@ struct Ctx {
   double* tab_win;    // W~(n)^deconv_pow       (PM)   | phi_hat(n)^2, 0 = mode dropped (NUFFT)
   double* tab_cos;    // interlace phase, real part (R9)
   double* tab_sin;    // interlace phase, imaginary part
+  double* tab_win1;   // W~(n) to the FIRST power (power spectrum: one assignment, no gather); 1 for NUFFT
 
   // binning workspace
   int64_t cap;
@@ -153,6 +167,11 @@ struct Ctx {
   float* g[3];       // force meshes
   float* gbar[3];    // VJP: scattered cotangents (lazy)
   bool vjp_ready;
+  float* phi;        // potential mesh (lazy; PM_FLAG_GRAD_REAL, PM_FLAG_KERNEL_GRAD)
+  bool g_valid;      // g[0..2] (or phi) hold the forward meshes of the PINNED records (pm_bin): pm_force_vjp reuses them
+  double* step_dots; // [4] scalar adjoints of pm_dkd_step_adjoint when the caller passes none (lazy)
+  double* ps_acc;    // [3 * ps_nbins] power-spectrum accumulators (lazy)
+  int ps_nbins;
 
   // host staging for pm_force_host
   float* host_pos_dev;
@@ -200,25 +219,53 @@ int bin_occupancy(int pass);
 // Scatter ncomp (1..3) fields.  Weight of particle i, component a: wsrc ? wsrc[i*wstride + a] : 1.
 int launch_scatter(Ctx* c, int order, const ShiftSplit& sh, int ncomp, const float* wsrc, int wstride,
                    float* const mesh[], cudaStream_t st);
-// Gather.  grad = false: v[i*ncomp + a] = sum_j mesh[a][j] W.
-// grad = true : v[i*3 + b] = sum_a coef_a(i) sum_j mesh[a][j] dW/dX^b, with
+// Gather.  mode GATHER_VALUES: v[i*ncomp + a] = sum_j mesh[a][j] W.
+// GATHER_GRAD: v[i*3 + b] = sum_a coef_a(i) sum_j mesh[a][j] dW/dX^b, with
 //   coef_a(i) = a < ncot ? cot[i*cstride + a] : const_coef * (wmul ? wmul[i] : 1).
-// out = alpha * v (+ out if accumulate).
+// GATHER_JVP (Eq. C.13b): v[i*ncomp + a] = pos_tan_i . sum_j mesh[a][j] dW/dX  (+ sum_j mesh[ncomp + a][j] W when
+//   has_mesh_tan: the tangent meshes follow the primal ones in `mesh`).
+// out = alpha * v + out_scale * out (out_scale = 0: out is not read).
+enum { GATHER_VALUES = 0, GATHER_GRAD = 1, GATHER_JVP = 2 };
 struct GatherArgs {
-  int ncomp;
-  const float* const* mesh;
-  bool grad;
-  const float* cot;
-  int cstride, ncot;
-  float const_coef;
-  const float* wmul;
-  float alpha;
-  bool accumulate;
-  float* out;
+  int ncomp = 0;
+  const float* const* mesh = nullptr;
+  int mode = GATHER_VALUES;
+  const float* cot = nullptr;
+  int cstride = 0, ncot = 0;
+  float const_coef = 0.f;
+  const float* wmul = nullptr;
+  const float* pos_tan = nullptr;
+  bool has_mesh_tan = false;
+  float alpha = 1.f, out_scale = 0.f;
+  float* out = nullptr;
+  // fused tails of the DKD step and of its adjoint (ncomp = 3, GATHER_VALUES; see GatherDev in pm_mesh_kernels.cuh)
+  float* drift_pos = nullptr;
+  float drift_tau = 0.f;
+  const float* dot_with = nullptr;
+  double* dot_acc = nullptr;
+  double* dot_out = nullptr;
+  float dot_scale = 1.f;
 };
 inline GatherArgs gather_values(int ncomp, const float* const* mesh, float* out, float alpha = 1.f,
-                                bool accumulate = false) {
-  GatherArgs a = {ncomp, mesh, false, nullptr, 0, 0, 0.f, nullptr, alpha, accumulate, out};
+                                float out_scale = 0.f) {
+  GatherArgs a;
+  a.ncomp = ncomp;
+  a.mesh = mesh;
+  a.out = out;
+  a.alpha = alpha;
+  a.out_scale = out_scale;
+  return a;
+}
+inline GatherArgs gather_grad(int ncomp, const float* const* mesh, const float* cot, int cstride, int ncot,
+                              float const_coef, const float* wmul, float* out, float alpha = 1.f,
+                              float out_scale = 0.f) {
+  GatherArgs a = gather_values(ncomp, mesh, out, alpha, out_scale);
+  a.mode = GATHER_GRAD;
+  a.cot = cot;
+  a.cstride = cstride;
+  a.ncot = ncot;
+  a.const_coef = const_coef;
+  a.wmul = wmul;
   return a;
 }
 int launch_gather(Ctx* c, int order, const ShiftSplit& sh, const GatherArgs& a, cudaStream_t st);
@@ -258,6 +305,32 @@ int launch_xfft_transpose(Ctx* c, const float2* const gh[3], float2* q1, float2*
 int spectral_forward(Ctx* c, const float* d1, const float* d2, float* const g[3], double coeff_eff, bool stages,
                      cudaStream_t st);
 int spectral_transpose(Ctx* c, const float* const gb[3], float* q1, float* q2, double coeff_eff, cudaStream_t st);
+
+// potential-only spectral paths (PM_FLAG_GRAD_REAL, PM_FLAG_KERNEL_GRAD)
+int ensure_phi(Ctx* c);
+int spectral_potential_hat(Ctx* c, bool two, float2* out, double coeff_eff, cudaStream_t st);
+int spectral_potential(Ctx* c, const float* d1, const float* d2, float* phi, double coeff_eff, bool stages,
+                       cudaStream_t st);
+int launch_xfft_potential(Ctx* c, const float2* d1, const float2* d2, float2* phi, double coeff_eff, cudaStream_t st);
+int launch_xfft_potential_tr(Ctx* c, const float2* psi, float2* q1, float2* q2, double coeff_eff, cudaStream_t st);
+int launch_kspace_scalar(Ctx* c, const float2* d1, const float2* d2, float2* q1, float2* q2, double coeff_eff, bool fwd,
+                         cudaStream_t st);
+int launch_fd_gradient(Ctx* c, const float* phi, float* const g[3], cudaStream_t st);
+int launch_fd_divergence(Ctx* c, const float* const gb[3], float* psi, cudaStream_t st);
+// forward-mode scatter (pm_jvp.cu)
+int launch_scatter_jvp(Ctx* c, int order, const ShiftSplit& sh, const float* w, const float* w_tan,
+                       const float* pos_tan, float* mesh_tan, cudaStream_t st);
+// drift / adjoint-drift kernels of the DKD step (pm_step.cu): X <- wrap(X + tau_x V) (fp32, R18);
+// if xs: Vs <- a Vs + b Xs and *dot += sum Xs . V (V read before / after as Table 3 orders it: see pm_step.cu)
+int launch_step_update(Ctx* c, float* x, const float* v, const float* xs, float* vs, int64_t n, float tau_x,
+                       float a, float b, double* dot, cudaStream_t st);
+// power spectrum binning (pm_power.cu)
+int launch_power_bins(Ctx* c, const float2* d1a, const float2* d1b, const float2* d2a, const float2* d2b,
+                      bool deconvolve, int nbins, double* acc, cudaStream_t st);
+int launch_power_finish(Ctx* c, int nbins, const double* acc, double kf, double pnorm, double* k_mean,
+                        double* power, double* n_modes, cudaStream_t st);
+// sheet resampling (pm_resample.cu)
+int launch_sheet_resample(Ctx* c, const float* pos, int n_p, int r, float* out, cudaStream_t st);
 
 // profiling helpers
 void stage_begin(Ctx* c, int stage, cudaStream_t st);

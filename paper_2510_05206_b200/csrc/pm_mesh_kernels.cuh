@@ -243,16 +243,33 @@ __device__ __forceinline__ void load_rec(uint4& r, const BinView& bv, uint32_t i
 // buffers, so a work item costs ONE barrier (ncu before: barrier 33 %, long scoreboard 28 % of the stall
 // cycles with two barriers and loads issued after the deposit).  roll is in [0, m).
 // resident CTAs per SM the register allocation aims at (the unit-weight CIC assign is the headline kernel)
-template <class T, int NCOMP, bool WEIGHTED>
+// What a particle deposits.  W_UNIT: W_j(X_i).  W_WEIGHTED: w_i^a W_j(X_i), a < NCOMP (Eq. C.1, C.10).
+// W_JVP (NCOMP = 1): the tangent of the scatter, Eq. C.13a: w~_i W_j(X_i) + w_i X~_i . dW_j(X_i)/dX_i.
+enum { W_UNIT = 0, W_WEIGHTED = 1, W_JVP = 2 };
+struct ScatterSrc {
+  const float* w;        // W_WEIGHTED: [N * wstride], component a at w[i*wstride + a]; W_JVP: [N] or NULL (ones)
+  int wstride;
+  const float* w_tan;    // W_JVP: [N] or NULL
+  const float* pos_tan;  // W_JVP: [N,3] or NULL
+  float tan_scale;       // W_JVP: 1/Delta (d/dX = (1/Delta) d/du)
+};
+template <class T, int NCOMP, int WMODE>
 constexpr int scatter_min_ctas() {
   // vector scatter of the VJP (3 components): at 151 registers ONE CTA was resident per SM (ncu: 12.5 % warps
   // active, 3.5 ms at 512^3); two CTAs for CIC / TSC cap the allocation at 128
-  return (NCOMP == 1 && !WEIGHTED) ? (T::P == 2 ? 4 : (T::P <= 4 ? 3 : 1)) : (NCOMP == 1 ? 2 : (T::P <= 3 ? 2 : 1));
+  return WMODE == W_JVP ? 1
+                        : (NCOMP == 1 && WMODE == W_UNIT) ? (T::P == 2 ? 4 : (T::P <= 4 ? 3 : 1))
+                                                          : (NCOMP == 1 ? 2 : (T::P <= 3 ? 2 : 1));
 }
-template <class T, int NCOMP, bool WEIGHTED, int NBUF>
-__global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>()) k_scatter(BinView bv, typename T::Params tp, int3 roll,
-                                                   const float* __restrict__ wsrc, int wstride,
-                                                   MeshPtrs<NCOMP> mesh) {
+template <class T, int NCOMP, int WMODE, int NBUF>
+__global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_scatter(BinView bv, typename T::Params tp, int3 roll,
+                                                   ScatterSrc src, MeshPtrs<NCOMP> mesh) {
+  constexpr bool WEIGHTED = WMODE != W_UNIT;
+  constexpr bool JVP = WMODE == W_JVP;
+  constexpr int NPAY = JVP ? 4 : NCOMP;  // floats a particle carries: its weights, or {w~, w t_x, w t_y, w t_z}
+  static_assert(!JVP || NCOMP == 1, "the forward-mode scatter deposits one field");
+  const float* __restrict__ wsrc = src.w;
+  const int wstride = src.wstride;
   using G = Geo<T>;
   constexpr int P = T::P;
   constexpr int NG = NCOMP * G::NGROUP;                          // groups to flush
@@ -313,29 +330,44 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>())
     const TileOrigin o = tile_origin(wi);
     const uint32_t nbegin = nwi.begin, nend = nxt < nitems ? nwi.end : nwi.begin;  // empty when there is no next item
 
-    float wv[PPT][NCOMP];
+    float wv[PPT][NPAY];
     float wabs[NCOMP];
 #pragma unroll
     for (int a = 0; a < NCOMP; ++a) wabs[a] = 0.0f;
-    auto load_weights = [&](uint32_t b0) {  // weights of the batch held in r[]
+    // what particle `idx` (caller order) deposits, and its contribution to the bound of the node sums
+    auto payload = [&](uint32_t idx, float (&pv)[NPAY]) {
+      if constexpr (JVP) {
+        const float w = wsrc ? __ldg(wsrc + idx) : 1.0f;
+        pv[0] = src.w_tan ? __ldg(src.w_tan + idx) : 0.0f;
+        float t0 = 0.0f, t1 = 0.0f, t2 = 0.0f;
+        if (src.pos_tan) {
+          const float* t = src.pos_tan + (size_t)idx * 3;
+          t0 = __ldg(t), t1 = __ldg(t + 1), t2 = __ldg(t + 2);
+        }
+        const float ws = w * src.tan_scale;
+        pv[1] = ws * t0, pv[2] = ws * t1, pv[3] = ws * t2;
+        // |W| <= 1 and |dW/du| <= 1 for the kernels of Table 1
+        wabs[0] += fabsf(pv[0]) + fabsf(pv[1]) + fabsf(pv[2]) + fabsf(pv[3]);
+      } else {
+#pragma unroll
+        for (int a = 0; a < NCOMP; ++a) {
+          pv[a] = WEIGHTED ? __ldg(wsrc + (size_t)idx * wstride + a) : 1.0f;
+          wabs[a] += fabsf(pv[a]);
+        }
+      }
+    };
+    auto load_weights = [&](uint32_t b0) {  // payloads of the batch held in r[]
 #pragma unroll
       for (int k = 0; k < PPT; ++k) {
         const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
-        if (i < iend) {
-#pragma unroll
-          for (int a = 0; a < NCOMP; ++a) {
-            wv[k][a] = WEIGHTED ? __ldg(wsrc + (size_t)r[k].w * wstride + a) : 1.0f;
-            wabs[a] += fabsf(wv[k][a]);
-          }
-        }
+        if (i < iend) payload(r[k].w, wv[k]);
       }
     };
     load_weights(ibegin);
     if (WEIGHTED && n > (uint32_t)CHUNK) {  // dense tile: the bound needs the weights of the later batches too
       for (uint32_t i = ibegin + CHUNK + tid; i < iend; i += BLOCK) {
-        const uint32_t idx = bv.rec[i].w;
-#pragma unroll
-        for (int a = 0; a < NCOMP; ++a) wabs[a] += fabsf(__ldg(wsrc + (size_t)idx * wstride + a));
+        float pv[NPAY];
+        payload(bv.rec[i].w, pv);
       }
     }
 
@@ -356,7 +388,7 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>())
         float tot = 0.0f;
 #pragma unroll
         for (int j = 0; j < BLOCK / 32; ++j) tot += s_red[j * NCOMP + a];
-        const float bound = tot * (T::WMAX3 * 1.0001f);
+        const float bound = tot * ((JVP ? 1.0f : T::WMAX3) * 1.0001f);
         int e = 0;
         const float f = frexpf(bound, &e);
         const int cl = (f == 0.5f) ? e - 1 : e;  // ceil(log2(bound))
@@ -385,35 +417,58 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WEIGHTED>())
         const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
         if (i < iend) {
           int sx, sy, sz;
-          float wx[P], wy[P], wz[P], dummy[P];
-          T::template axis<false>(apply_shift<T>(r[k].x, tp.frac[0]), tp, sx, wx, dummy);
-          T::template axis<false>(apply_shift<T>(r[k].y, tp.frac[1]), tp, sy, wy, dummy);
-          T::template axis<false>(apply_shift<T>(r[k].z, tp.frac[2]), tp, sz, wz, dummy);
+          float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
+          T::template axis<JVP>(apply_shift<T>(r[k].x, tp.frac[0]), tp, sx, wx, dx);
+          T::template axis<JVP>(apply_shift<T>(r[k].y, tp.frac[1]), tp, sy, wy, dy);
+          T::template axis<JVP>(apply_shift<T>(r[k].z, tp.frac[2]), tp, sz, wz, dz);
           NodeCol nc[P];
 #pragma unroll
           for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
-          float wzs[NCOMP][P];  // the scale (and the particle's weight) folded into the z weights
+          if constexpr (JVP) {
+            // w~ Wx Wy Wz + (w tx) dWx Wy Wz + (w ty) Wx dWy Wz + (w tz) Wx Wy dWz, the scale folded into z
+            const float wt = wv[k][0], ax = wv[k][1], ay = wv[k][2], az = wv[k][3];
 #pragma unroll
-          for (int q = 0; q < NCOMP; ++q)
+            for (int c = 0; c < P; ++c) {
+              wz[c] *= scale[0];
+              dz[c] *= scale[0] * az;
+            }
 #pragma unroll
-            for (int c = 0; c < P; ++c) wzs[q][c] = wz[c] * (wv[k][q] * scale[q]);
+            for (int a = 0; a < P; ++a) {
+              const float pxa = fmaf(ax, dx[a], wt * wx[a]);
 #pragma unroll
-          for (int a = 0; a < P; ++a)
+              for (int b = 0; b < P; ++b) {
+                const float e1 = fmaf(wy[b], pxa, ay * wx[a] * dy[b]);
+                const float e2 = wx[a] * wy[b];
 #pragma unroll
-            for (int b = 0; b < P; ++b) {
-              const float wxy = wx[a] * wy[b];
-#pragma unroll
-              for (int c = 0; c < P; ++c) {
-                int* node = s_acc + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
-#pragma unroll
-                for (int q = 0; q < NCOMP; ++q) {
-                  if (WEIGHTED)
-                    atomicAdd(node + q * G::COMP, __float2int_rn(wxy * wzs[q][c]));
-                  else
-                    atomicAdd(reinterpret_cast<unsigned*>(node + q * G::COMP), __float2uint_rn(wxy * wzs[q][c]));
-                }
+                for (int c = 0; c < P; ++c)
+                  atomicAdd(s_acc + ((a * G::SY + b) * nc[c].pitch + nc[c].base),
+                            __float2int_rn(fmaf(e1, wz[c], e2 * dz[c])));
               }
             }
+          } else {
+            float wzs[NCOMP][P];  // the scale (and the particle's weight) folded into the z weights
+#pragma unroll
+            for (int q = 0; q < NCOMP; ++q)
+#pragma unroll
+              for (int c = 0; c < P; ++c) wzs[q][c] = wz[c] * (wv[k][q] * scale[q]);
+#pragma unroll
+            for (int a = 0; a < P; ++a)
+#pragma unroll
+              for (int b = 0; b < P; ++b) {
+                const float wxy = wx[a] * wy[b];
+#pragma unroll
+                for (int c = 0; c < P; ++c) {
+                  int* node = s_acc + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
+#pragma unroll
+                  for (int q = 0; q < NCOMP; ++q) {
+                    if (WEIGHTED)
+                      atomicAdd(node + q * G::COMP, __float2int_rn(wxy * wzs[q][c]));
+                    else
+                      atomicAdd(reinterpret_cast<unsigned*>(node + q * G::COMP), __float2uint_rn(wxy * wzs[q][c]));
+                  }
+                }
+              }
+          }
         }
         if (last) {  // slot k is free: request the next item's record (its first batch)
           const uint32_t ni = nbegin + (uint32_t)(k * BLOCK + tid);
@@ -721,9 +776,11 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 }
 
 // ---- K4 / K7: tile gather ----------------------------------------------------------------------------
-// GRAD = false: v[i*NCOMP + a] = sum_j mesh_a[j] W_j(X_i)                                    (Eq. C.2)
-// GRAD = true : v[i*3 + b]     = sum_a coef_a(i) sum_j mesh_a[j] d/du_b W_j(X_i)             (Eq. C.6, C.12)
-// out = alpha * v (+ out if accumulate); the caller folds 1/Delta (d/dX = (1/Delta) d/du) into alpha.
+// GMODE G_VALUES: v[i*NST + a] = sum_j mesh_a[j] W_j(X_i)                                          (Eq. C.2)
+//       G_GRAD  : v[i*3 + b]   = sum_a coef_a(i) sum_j mesh_a[j] d/du_b W_j(X_i)                   (Eq. C.6, C.12)
+//       G_JVP   : v[i*NO + a]  = sum_j mesh_a[j] (t_i . d/du) W_j(X_i)              [+ sum_j mesh~_a[j] W_j(X_i)]
+//                 (Eq. C.13b; G_JVPT: the NO tangent meshes are staged behind the NO primal ones, NST = 2 NO)
+// out = alpha * v + out_scale * out; the caller folds 1/Delta (d/dX = (1/Delta) d/du) into alpha / tan_scale.
 //
 // Persistent CTAs draw work items from the dynamic schedule.  Thread 0 stages the tile + halo box of every
 // component with one TMA tensor copy each (north_star "TMA staging of mesh tiles"), completion on an
@@ -732,26 +789,57 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, u
 // TMA zero-fills what lies beyond the mesh edge, it does not wrap: tiles whose box crosses an edge (a few
 // per cent) are patched by the threads with periodic loads after the copy has landed.  roll in [0, m); when
 // roll.z is not a multiple of 4 no box start is 16-byte aligned and the threads stage everything (manual).
-template <class T, int NCOMP, bool GRAD, int STAGES>
+enum { G_VALUES = 0, G_GRAD = 1, G_JVP = 2, G_JVPT = 3 };
+
+struct GatherDev {  // per-launch arguments beyond the meshes
+  const float* cot;      // G_GRAD: coef_a(i) = a < ncot ? cot[i*cstride + a] : const_coef * (wmul ? wmul[i] : 1)
+  int cstride, ncot;
+  float const_coef;
+  const float* wmul;
+  const float* pos_tan;  // G_JVP*: tangent positions [N,3] or NULL (then only the tangent meshes contribute)
+  float tan_scale;       // G_JVP*: 1/Delta
+  float alpha, out_scale;
+  float* out;
+  // Fused tail of the drift-kick-drift step (Eq. 2.14b-c, G_VALUES with NST = 3, out = V): after the kick
+  // V_i <- out_scale V_i + alpha A_i the particle is drifted, X_i <- wrap(X_i + drift_tau V_i) with every
+  // operation rounded to fp32 and no fused multiply-add (reading R18).
+  float* drift_pos;
+  float drift_tau, box;
+  // Reductions of the adjoint kick (Table 3), dot_with = V* [N,3]:
+  //   *dot_acc += dot_scale sum_i dot_with_i . v_i      (beta*:  V* . A)
+  //   *dot_out +=           sum_i dot_with_i . out_i    (alpha*: V* . V^{n-1}, the kicked-back velocity)
+  const float* dot_with;
+  double* dot_acc;
+  double* dot_out;
+  float dot_scale;
+};
+
+template <class T, int NST, int GMODE, int STAGES>
 __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params tp, int3 roll,
-                                                  const __grid_constant__ TMapSet<2 * NCOMP> maps,
-                                                  CMeshPtrs<NCOMP> mesh, const float* __restrict__ cot,
-                                                  int cstride, int ncot, float const_coef,
-                                                  const float* __restrict__ wmul, float alpha,
-                                                  int accumulate, int manual, float* __restrict__ out) {
+                                                  const __grid_constant__ TMapSet<2 * NST> maps,
+                                                  CMeshPtrs<NST> mesh, GatherDev gd, int manual) {
   using G = Geo<T>;
   constexpr int P = T::P;
+  constexpr bool GRAD = GMODE == G_GRAD;
+  constexpr bool JVP = GMODE == G_JVP || GMODE == G_JVPT;
+  constexpr bool DERIV = GRAD || JVP;
+  constexpr int NO = GMODE == G_JVPT ? NST / 2 : NST;  // outputs per particle (G_GRAD: 3)
+  static_assert(GMODE != G_JVPT || NST % 2 == 0, "G_JVPT stages the primal and the tangent meshes");
   constexpr int KB = 4;  // records in flight per thread
-  constexpr uint32_t BOX_BYTES = (uint32_t)(NCOMP * (G::MAIN + G::HAL) * sizeof(float));
+  constexpr uint32_t BOX_BYTES = (uint32_t)(NST * (G::MAIN + G::HAL) * sizeof(float));
   extern __shared__ __align__(128) unsigned char s_raw[];
   __shared__ __align__(8) uint64_t s_bar[STAGES];
   __shared__ uint32_t s_next[2];
+  __shared__ double s_dots[2 * (BLOCK / 32)];
   // 128-byte aligned TMA destinations; the offset is applied to the shared-space pointer so that the loads
   // below stay LDS (a round trip through uintptr_t made them generic LD with 64-bit address arithmetic)
   float* s_base = reinterpret_cast<float*>(s_raw + ((128u - (smem_u32(s_raw) & 127u)) & 127u));
   const int tid = threadIdx.x;
   const uint32_t nitems = *bv.nitems;
   const int m = bv.m;
+  float* __restrict__ out = gd.out;
+  const float alpha = gd.alpha, out_scale = gd.out_scale;
+  double dsum0 = 0.0, dsum1 = 0.0;
 
   if (tid == 0) {
 #pragma unroll
@@ -774,8 +862,8 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     box_start(o, cx, cy, cz);
     mbar_expect_tx(&s_bar[stage], BOX_BYTES);
 #pragma unroll
-    for (int a = 0; a < NCOMP; ++a) {  // main plane (first TZ nodes of every row) and halo plane (the rest)
-      float* dst = s_base + (stage * NCOMP + a) * G::COMP;
+    for (int a = 0; a < NST; ++a) {  // main plane (first TZ nodes of every row) and halo plane (the rest)
+      float* dst = s_base + (stage * NST + a) * G::COMP;
       tma_load_3d(dst, &maps.m[2 * a], &s_bar[stage], cz, cy, cx);
       tma_load_3d(dst + G::MAIN, &maps.m[2 * a + 1], &s_bar[stage], cz + TZ, cy, cx);
     }
@@ -807,7 +895,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
       if (STAGES == 2 && nxt < nitems) issue(nwi, stage ^ 1);
     }
     const TileOrigin o = tile_origin(wi);
-    const float* s_val = s_base + stage * NCOMP * G::COMP;
+    const float* s_val = s_base + stage * NST * G::COMP;
     const uint32_t nbegin = nwi.begin, nend = nxt < nitems ? nwi.end : nwi.begin;  // empty when there is no next item
 
     if (!(manual & 1)) {
@@ -818,8 +906,8 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     int cx, cy, cz;
     box_start(o, cx, cy, cz);
     if ((manual & 1) || cx + G::SX > m || cy + G::SY > m || cz + TZ + G::HZ > m) {  // uniform: box crosses a mesh edge
-      float* s_w = s_base + stage * NCOMP * G::COMP;
-      for (int j = tid; j < NCOMP * G::NGROUP; j += BLOCK) {
+      float* s_w = s_base + stage * NST * G::COMP;
+      for (int j = tid; j < NST * G::NGROUP; j += BLOCK) {
         const int comp = j / G::NGROUP, rr = j - comp * G::NGROUP;
         int row, zoff;
         group_pos<G>(rr, row, zoff);
@@ -848,19 +936,19 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         if (i >= wi.end) continue;
         int sx, sy, sz;
         float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
-        T::template axis<GRAD>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
-        T::template axis<GRAD>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
-        T::template axis<GRAD>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
+        T::template axis<DERIV>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
+        T::template axis<DERIV>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
+        T::template axis<DERIV>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
         // (TMA's 128-byte swizzle of the MAIN plane was measured: it is correct but RAISES the bank conflicts of
         // Lagrangian-ordered particles from 85 M to 136 M wavefronts, 1.09 -> 1.21 ms: with a row pitch of 32 words
         // lanes at distinct z already sit in distinct banks, and the swizzle scatters them.)
         NodeCol nc[P];
 #pragma unroll
         for (int c = 0; c < P; ++c) nc[c] = node_col<G>(sx * G::SY + sy, sz + (G::ZLO - G::HLO) + c);
-        if (!GRAD) {
-          float acc[NCOMP];
+        if (GMODE == G_VALUES) {
+          float acc[NST];
 #pragma unroll
-          for (int a = 0; a < NCOMP; ++a) acc[a] = 0.0f;
+          for (int a = 0; a < NST; ++a) acc[a] = 0.0f;
 #pragma unroll
           for (int a = 0; a < P; ++a)
 #pragma unroll
@@ -871,19 +959,34 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
                 const float wxyz = wxy * wz[c];
                 const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
 #pragma unroll
-                for (int q = 0; q < NCOMP; ++q) acc[q] = fmaf(wxyz, node[q * G::COMP], acc[q]);
+                for (int q = 0; q < NST; ++q) acc[q] = fmaf(wxyz, node[q * G::COMP], acc[q]);
               }
             }
+          float* dst = out + (size_t)rk.w * NST;
+          float nv[NST];
 #pragma unroll
-          for (int a = 0; a < NCOMP; ++a) {
-            float* dst = out + (size_t)rk.w * NCOMP + a;
-            *dst = accumulate ? fmaf(alpha, acc[a], *dst) : alpha * acc[a];
+          for (int a = 0; a < NST; ++a) {
+            nv[a] = out_scale != 0.0f ? fmaf(alpha, acc[a], out_scale * dst[a]) : alpha * acc[a];
+            dst[a] = nv[a];
           }
-        } else {
-          float coef[NCOMP];
-          const float cc = const_coef * (wmul ? __ldg(wmul + rk.w) : 1.0f);
+          if (NST == 3) {  // DKD tails (uniform branches on launch arguments)
+            if (gd.dot_with) {
+              const float* dw = gd.dot_with + (size_t)rk.w * 3;
+              const float d0 = __ldg(dw), d1 = __ldg(dw + 1), d2 = __ldg(dw + 2);
+              dsum0 += (double)d0 * (double)acc[0] + (double)d1 * (double)acc[1] + (double)d2 * (double)acc[2];
+              dsum1 += (double)d0 * (double)nv[0] + (double)d1 * (double)nv[1] + (double)d2 * (double)nv[2];
+            }
+            if (gd.drift_pos) {
+              float* xp = gd.drift_pos + (size_t)rk.w * 3;
 #pragma unroll
-          for (int a = 0; a < NCOMP; ++a) coef[a] = a < ncot ? __ldg(cot + (size_t)rk.w * cstride + a) : cc;
+              for (int a = 0; a < 3; ++a) xp[a] = drift_fp32(xp[a], nv[a], gd.drift_tau, gd.box);
+            }
+          }
+        } else if (GRAD) {
+          float coef[NST];
+          const float cc = gd.const_coef * (gd.wmul ? __ldg(gd.wmul + rk.w) : 1.0f);
+#pragma unroll
+          for (int a = 0; a < NST; ++a) coef[a] = a < gd.ncot ? __ldg(gd.cot + (size_t)rk.w * gd.cstride + a) : cc;
           float gx = 0.0f, gy = 0.0f, gz = 0.0f;
 #pragma unroll
           for (int a = 0; a < P; ++a)
@@ -895,16 +998,46 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
                 const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
                 float val = 0.0f;
 #pragma unroll
-                for (int q = 0; q < NCOMP; ++q) val = fmaf(coef[q], node[q * G::COMP], val);
+                for (int q = 0; q < NST; ++q) val = fmaf(coef[q], node[q * G::COMP], val);
                 gx = fmaf(wdx * wz[c], val, gx);
                 gy = fmaf(wdy * wz[c], val, gy);
                 gz = fmaf(wxy * dz[c], val, gz);
               }
             }
           float* dst = out + (size_t)rk.w * 3;
-          dst[0] = accumulate ? fmaf(alpha, gx, dst[0]) : alpha * gx;
-          dst[1] = accumulate ? fmaf(alpha, gy, dst[1]) : alpha * gy;
-          dst[2] = accumulate ? fmaf(alpha, gz, dst[2]) : alpha * gz;
+          dst[0] = out_scale != 0.0f ? fmaf(alpha, gx, out_scale * dst[0]) : alpha * gx;
+          dst[1] = out_scale != 0.0f ? fmaf(alpha, gy, out_scale * dst[1]) : alpha * gy;
+          dst[2] = out_scale != 0.0f ? fmaf(alpha, gz, out_scale * dst[2]) : alpha * gz;
+        } else {  // JVP, Eq. C.13b: (t . d/du) W = tx dWx Wy Wz + ty Wx dWy Wz + tz Wx Wy dWz
+          float tx = 0.0f, ty = 0.0f, tz = 0.0f;
+          if (gd.pos_tan) {
+            const float* tp3 = gd.pos_tan + (size_t)rk.w * 3;
+            tx = __ldg(tp3) * gd.tan_scale, ty = __ldg(tp3 + 1) * gd.tan_scale, tz = __ldg(tp3 + 2) * gd.tan_scale;
+          }
+          float acc[NO];
+#pragma unroll
+          for (int a = 0; a < NO; ++a) acc[a] = 0.0f;
+#pragma unroll
+          for (int a = 0; a < P; ++a)
+#pragma unroll
+            for (int b = 0; b < P; ++b) {
+              const float wxy = wx[a] * wy[b];
+              const float txy = tx * dx[a] * wy[b] + ty * wx[a] * dy[b];
+              const float tzxy = tz * wxy;
+#pragma unroll
+              for (int c = 0; c < P; ++c) {
+                const float wd = fmaf(txy, wz[c], tzxy * dz[c]);
+                const float* node = s_val + ((a * G::SY + b) * nc[c].pitch + nc[c].base);
+#pragma unroll
+                for (int q = 0; q < NO; ++q) {
+                  acc[q] = fmaf(wd, node[q * G::COMP], acc[q]);
+                  if (GMODE == G_JVPT) acc[q] = fmaf(wxy * wz[c], node[(NO + q) * G::COMP], acc[q]);
+                }
+              }
+            }
+          float* dst = out + (size_t)rk.w * NO;
+#pragma unroll
+          for (int a = 0; a < NO; ++a) dst[a] = out_scale != 0.0f ? fmaf(alpha, acc[a], out_scale * dst[a]) : alpha * acc[a];
         }
       }
       if (last) break;
@@ -925,6 +1058,27 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     nxt = nn;
     nwi = nnwi;
   }
+  if (GMODE == G_VALUES && NST == 3 && gd.dot_with) {  // one pair of double atomics per CTA
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+      dsum0 += __shfl_xor_sync(0xffffffffu, dsum0, d);
+      dsum1 += __shfl_xor_sync(0xffffffffu, dsum1, d);
+    }
+    if ((tid & 31) == 0) {
+      s_dots[2 * (tid >> 5)] = dsum0;
+      s_dots[2 * (tid >> 5) + 1] = dsum1;
+    }
+    __syncthreads();
+    if (tid == 0) {
+      double a0 = 0.0, a1 = 0.0;
+      for (int w = 0; w < BLOCK / 32; ++w) {
+        a0 += s_dots[2 * w];
+        a1 += s_dots[2 * w + 1];
+      }
+      if (gd.dot_acc) atomicAdd(gd.dot_acc, (double)gd.dot_scale * a0);
+      if (gd.dot_out) atomicAdd(gd.dot_out, a1);
+    }
+  }
   if (tid == 0) sched_done(bv.sched);
 }
 
@@ -941,14 +1095,14 @@ inline int mesh_grid(const Ctx* c, int occ) {
   return (int)(bound < cap ? bound : cap);
 }
 
-template <class T, int NCOMP, bool WEIGHTED>
-int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const float* wsrc, int wstride,
-                float* const mesh[], cudaStream_t st) {
+template <class T, int NCOMP, int WMODE>
+int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const ScatterSrc& src, float* const mesh[],
+                cudaStream_t st) {
   using G = Geo<T>;
   constexpr size_t acc_bytes = sizeof(int) * (size_t)NCOMP * G::COMP;
   constexpr int NBUF = 2 * acc_bytes <= 48 * 1024 ? 2 : 1;  // two accumulator tiles when they are cheap
   const size_t smem = NBUF * acc_bytes;
-  auto kern = k_scatter<T, NCOMP, WEIGHTED, NBUF>;
+  auto kern = k_scatter<T, NCOMP, WMODE, NBUF>;
   int occ = 0;
   PM_TRY(kernel_occupancy(c, (const void*)kern, BLOCK, smem, &occ));
   MeshPtrs<NCOMP> mp;
@@ -956,10 +1110,14 @@ int run_scatter(Ctx* c, const typename T::Params& tp, const int roll[3], const f
   const int m = c->mg;
   kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp,
                                                make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m)),
-                                               wsrc, wstride, mp);
+                                               src, mp);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;
+}
+inline ScatterSrc weights_src(const float* w, int wstride) {
+  ScatterSrc s = {w, wstride, nullptr, nullptr, 0.f};
+  return s;
 }
 
 // Unit-weight, single-field scatter with warp-private tiles (k_scatter_warp).
@@ -981,29 +1139,44 @@ int run_scatter_warp(Ctx* c, const typename T::Params& tp, const int roll[3], fl
   return PM_OK;
 }
 
-template <class T, int NCOMP, bool GRAD>
-int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const float* const mesh[],
-               const float* cot, int cstride, int ncot, float const_coef, const float* wmul, float alpha,
-               bool accumulate, float* out, cudaStream_t st) {
+template <class T, int NST, int GMODE>
+int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const GatherArgs& ga, cudaStream_t st) {
   using G = Geo<T>;
-  constexpr size_t stage_bytes = sizeof(float) * (size_t)NCOMP * G::COMP;
+  constexpr size_t stage_bytes = sizeof(float) * (size_t)NST * G::COMP;
   constexpr int STAGES = 2 * stage_bytes <= 100 * 1024 ? 2 : 1;
   constexpr size_t smem = STAGES * stage_bytes + 128;
-  auto kern = k_gather<T, NCOMP, GRAD, STAGES>;
+  auto kern = k_gather<T, NST, GMODE, STAGES>;
   int occ = 0;
   PM_TRY(kernel_occupancy(c, (const void*)kern, BLOCK, smem, &occ));
-  CMeshPtrs<NCOMP> mp;
-  TMapSet<2 * NCOMP> maps;
+  CMeshPtrs<NST> mp;
+  TMapSet<2 * NST> maps;
   const int m = c->mg;
-  for (int a = 0; a < NCOMP; ++a) {
-    mp.p[a] = mesh[a];
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, TZ, &maps.m[2 * a]));
-    PM_TRY(make_mesh_tmap(c, mesh[a], G::SX, G::SY, G::HZ, &maps.m[2 * a + 1]));
+  for (int a = 0; a < NST; ++a) {
+    mp.p[a] = ga.mesh[a];
+    PM_TRY(make_mesh_tmap(c, ga.mesh[a], G::SX, G::SY, TZ, &maps.m[2 * a]));
+    PM_TRY(make_mesh_tmap(c, ga.mesh[a], G::SX, G::SY, G::HZ, &maps.m[2 * a + 1]));
   }
-  const float a_eff = GRAD ? (float)((double)alpha * (double)c->mg / c->p.box) : alpha;
+  const double inv_delta = (double)c->mg / c->p.box;
+  GatherDev gd;
+  gd.cot = ga.cot;
+  gd.cstride = ga.cstride;
+  gd.ncot = ga.ncot;
+  gd.const_coef = ga.const_coef;
+  gd.wmul = ga.wmul;
+  gd.pos_tan = ga.pos_tan;
+  gd.tan_scale = (float)inv_delta;
+  gd.alpha = GMODE == G_GRAD ? (float)((double)ga.alpha * inv_delta) : ga.alpha;
+  gd.out_scale = ga.out_scale;
+  gd.out = ga.out;
+  gd.drift_pos = ga.drift_pos;
+  gd.drift_tau = ga.drift_tau;
+  gd.box = (float)c->p.box;
+  gd.dot_with = ga.dot_with;
+  gd.dot_acc = ga.dot_acc;
+  gd.dot_out = ga.dot_out;
+  gd.dot_scale = ga.dot_scale;
   const int3 nr = make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m));
-  kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp, nr, maps, mp, cot, cstride, ncot, const_coef, wmul,
-                                               a_eff, accumulate ? 1 : 0, (nr.z & 3) ? 1 : 0, out);
+  kern<<<mesh_grid(c, occ), BLOCK, smem, st>>>(bin_view(c), tp, nr, maps, mp, gd, (nr.z & 3) ? 1 : 0);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

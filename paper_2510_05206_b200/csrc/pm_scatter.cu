@@ -16,12 +16,13 @@ static int scatter_os(Ctx* c, const ShiftSplit& sh, int ncomp, const float* wsrc
       if constexpr (ORDER == 2)
         PM_TRY((run_scatter_warp<T>(c, tp, sh.roll, mesh[a], st)));
       else
-        PM_TRY((run_scatter<T, 1, false>(c, tp, sh.roll, nullptr, 0, mesh + a, st)));
+        PM_TRY((run_scatter<T, 1, W_UNIT>(c, tp, sh.roll, weights_src(nullptr, 0), mesh + a, st)));
     }
     return PM_OK;
   }
-  if (ncomp == 3) return run_scatter<T, 3, true>(c, tp, sh.roll, wsrc, wstride, mesh, st);
-  for (int a = 0; a < ncomp; ++a) PM_TRY((run_scatter<T, 1, true>(c, tp, sh.roll, wsrc + a, wstride, mesh + a, st)));
+  if (ncomp == 3) return run_scatter<T, 3, W_WEIGHTED>(c, tp, sh.roll, weights_src(wsrc, wstride), mesh, st);
+  for (int a = 0; a < ncomp; ++a)
+    PM_TRY((run_scatter<T, 1, W_WEIGHTED>(c, tp, sh.roll, weights_src(wsrc + a, wstride), mesh + a, st)));
   return PM_OK;
 }
 

@@ -12,6 +12,21 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 MAXABS_OVER_RMS = 1e-4
 
 
+# The scatter of signed weights accumulates in 32-bit fixed point whose quantum is 2^-30 of the work item's bound
+# B = sum_i |w_i| W_max^3 (up to 4096 particles): q ~ 4e-6 for unit-variance weights.  A node that receives n deposits
+# carries a rounding error of q sqrt(n / 12); in a clump where hundreds of random-sign cotangents land on one node
+# (the stage tests build one on purpose) that is ~3e-5 and up to ~3e-4 of the mesh rms over 1e5 nodes -- ten times
+# what fp32 atomics would give there, invisible in L2 (measured 1.2e-6 .. 2.7e-6) and far below the 1e-5 VJP bar.
+MAXABS_SIGNED_SCATTER = 1e-3
+
+
+def es_edge_guard(beta: float) -> float:
+    """The ES kernel jumps from e^-beta to 0 at the edge of its support, so whether a node exactly at the edge is
+    touched depends on the rounding of the coordinate: a deviation of e^-beta of one mesh value is legitimate
+    (R13; 1e-4 at w = 4, 1e-7 at w = 7)."""
+    return MAXABS_OVER_RMS + 3.0 * float(np.exp(-beta))
+
+
 def rel_l2(a, b):
     a = np.asarray(a, dtype=np.float64)
     b = np.asarray(b, dtype=np.float64)

@@ -12,7 +12,7 @@ from oracle import nufft_oracle as no
 from oracle import pm_oracle as po
 from pm_inputs import generators as gen
 
-from parity_util import check, record_error, rel_l2
+from parity_util import MAXABS_SIGNED_SCATTER, check, es_edge_guard, record_error, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -193,10 +193,14 @@ def test_nufft_interp_vjp_parity(pm, width, ncomp):
     pm.nufft_interp_vjp(ctx, [dev(meshes[a]) for a in range(ncomp)], dev(pos), dev(cot), fine_cot=fc, pos_cot=pc)
     refp = np.zeros((n, 3))
     for a in range(ncomp):
-        check(f"fine_cot{a}", fc[a], no.es_spread(pos, mf, box, w, beta, weights=cot[:, a]), 5e-6)
+        check(f"fine_cot{a}", fc[a], no.es_spread(pos, mf, box, w, beta, weights=cot[:, a]), 5e-6,
+              maxabs_tol=MAXABS_SIGNED_SCATTER)
         for b in range(3):
             refp[:, b] += cot[:, a] * no.es_interp(meshes[a], pos, box, w, beta, deriv_axis=b)
-    check("pos_cot", pc, refp, 5e-6)
+    # R13: the ES kernel's derivative ~ e^{-beta} / sqrt(1 - z^2) is unbounded at the support edge; a particle
+    # within ~1e-6 of it carries an O(1) relative error in that one weight (fp32 1 - z^2), visible in the max norm
+    # at the narrow widths (e^{-beta} = 1e-4 at w = 4) and invisible in L2: "parity unpinned" there
+    check("pos_cot", pc, refp, 5e-6, maxabs_tol=2e-3 if width <= 5 else 1e-4)
     pm.pm_destroy(ctx)
 
 
@@ -234,7 +238,8 @@ def test_nufft_force_parity(pm, sigma, eps, width):
     pos, c = gen.make_config_positions("cfg3", n_p=48)
     f = gpu_force(pm, nufft_params(pm, c["m"], c["box"], pos.shape[0], sigma=sigma, eps=eps, width=width), pos)
     ref = no.nufft_force(pos, c["m"], c["box"], sigma=sigma, eps=eps, width=width)
-    check(f"nufft_force/cfg3-48/sigma={sigma}/eps={eps}/w={width}", f, ref, 1e-5)
+    check(f"nufft_force/cfg3-48/sigma={sigma}/eps={eps}/w={width}", f, ref, 1e-5,
+          maxabs_tol=es_edge_guard(no.es_params(eps, sigma, width)[1]))
 
 
 def test_nufft_force_vjp_parity(pm):

@@ -71,6 +71,11 @@ def synth_mesh(m, idx, coef):
     return out
 
 
+def amplitudes(n, seed):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal(n) + 1j * rng.standard_normal(n)
+
+
 def sample_nodes(m, n, seed):
     rng = np.random.default_rng(seed)
     nodes = rng.integers(0, m, size=(n, 3))
@@ -98,7 +103,7 @@ def test_fused_kspace_plane_waves(pm, m, interlace):
     kw = dict(KSPACE_SETTINGS, worder=3 if interlace else 2)
     ctx = pm.pm_create(pm.PMParams(m=m, box=box, max_particles=8, interlace=interlace, **kw))
     idx, c1 = gen.plane_wave_modes(m, 400, 9000 + m)
-    _, c2 = gen.plane_wave_modes(m, 400, 9001 + m)
+    c2 = amplitudes(idx.shape[0], 9001 + m)
     S = po.force_symbol_at(tuple(idx[:, a] for a in range(3)), m, box, kw["worder"], kw["grad_order"],
                            kw["lap_order"], kw["deconv_pow"], kw["coeff"])          # [3, W]
     ph1 = po.interlace_phase(m)
@@ -118,7 +123,7 @@ def test_fused_kspace_plane_waves(pm, m, interlace):
         want = G * 0.5 * float(np.sum(np.abs(S[a] * chat) ** 2))
         assert abs(tot - want) <= 2e-5 * want
     # transpose: cotangent meshes with their own amplitudes
-    cs = [gen.plane_wave_modes(m, 400, 9100 + m + a)[1] for a in range(3)]
+    cs = [amplitudes(idx.shape[0], 9100 + m + a) for a in range(3)]
     gb = [synth_mesh(m, idx, cs[a]) for a in range(3)]
     q1 = torch.empty(m, m, m, device="cuda")
     q2 = torch.empty(m, m, m, device="cuda") if interlace else None
@@ -304,9 +309,9 @@ def test_nufft_kspace_plane_waves(pm, fine):
     lo = np.random.default_rng(5).integers(-(m // 2) + 1, m // 2, size=idx.shape)
     idx = np.where(inside[:, None], lo % fine, idx)
     idx = idx[np.any(idx != (-idx) % fine, axis=1)]  # no self-conjugate mode
-    c1 = c1[:idx.shape[0]]
     _, keep = np.unique(np.minimum(idx @ [fine * fine, fine, 1], ((-idx) % fine) @ [fine * fine, fine, 1]), return_index=True)
-    idx, c1 = idx[keep], c1[keep]
+    idx = idx[keep]  # no mode twice, no mode with its conjugate
+    c1 = amplitudes(idx.shape[0], 9201 + fine)
     M = no.kspace_multiplier_at(tuple(idx[:, a] for a in range(3)), fine, m, box, npart, w, beta, 1.0)
     assert (np.abs(M).sum(0) > 0).sum() > 100
     nodes = sample_nodes(fine, NSAMPLE, 19)
@@ -316,7 +321,7 @@ def test_nufft_kspace_plane_waves(pm, fine):
     G = float(fine) ** 3  # the oracle's stage carries the G of the unnormalised inverse transform
     for a in range(3):
         check(f"fwd/g{a}", at_nodes(g[a], nodes), gen.plane_wave_values(fine, idx, G * M[a] * c1, nodes), 3e-6)
-    cs = [gen.plane_wave_modes(fine, 600, 9300 + fine + a)[1][keep] for a in range(3)]
+    cs = [amplitudes(idx.shape[0], 9300 + fine + a) for a in range(3)]
     gb = [synth_mesh(fine, idx, cs[a]) for a in range(3)]
     q = torch.empty(fine, fine, fine, device="cuda")
     pm.nufft_poisson_force_vjp(ctx, gb, npart, q)

@@ -1,0 +1,366 @@
+"""GPU parity of the SURVEY 8(f) NEXT rows against their oracles:
+NEXT-1 drift-kick-drift step and its backward-in-time adjoint (oracle/dkd_oracle.py, Eq. 2.14, Table 3);
+NEXT-2 forward-mode rules of scatter / gather (pm_oracle.scatter_jvp / gather_jvp, Eq. C.13);
+NEXT-3 real-space finite-difference gradient (ONE inverse FFT; against the UNCHANGED pm_oracle.force) and the
+       ES kernel-gradient force (nufft_oracle.nufft_force(kernel_grad=True));
+NEXT-4 binned power spectrum and sheet resampling (oracle/analysis_oracle.py).
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import analysis_oracle as ao
+from oracle import dkd_oracle as dk
+from oracle import nufft_oracle as no
+from oracle import pm_oracle as po
+from pm_inputs import generators as gen
+
+from parity_util import MAXABS_SIGNED_SCATTER, check, es_edge_guard, record_error, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pm():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2510_05206_b200 as pm_
+
+    return pm_
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def params_of(pm, c, n, **over):
+    kw = dict(m=c["m"], box=c["box"], max_particles=n, worder=c.get("worder", 2), interlace=c.get("interlace", 0),
+              deconv_pow=c.get("deconv_pow", 2), grad_order=c.get("grad_order", 0), lap_order=c.get("lap_order", 0))
+    kw.update(over)
+    return pm.PMParams(**kw)
+
+
+def oracle_kw(c, **over):
+    kw = dict(worder=c.get("worder", 2), interlace=c.get("interlace", 0), grad_order=c.get("grad_order", 0),
+              lap_order=c.get("lap_order", 0), deconv_pow=c.get("deconv_pow", 2))
+    kw.update(over)
+    return kw
+
+
+def minimg(d, box):
+    return d - box * np.round(d / box)
+
+
+# ---- NEXT-3: real-space gradient ------------------------------------------------------------------------------
+@pytest.mark.parametrize("m,fused", [(32, True), (64, True), (64, False), (128, True)])
+@pytest.mark.parametrize("grad_order", [2, 4, 6])
+def test_real_gradient_kspace_stage(pm, m, fused, grad_order):
+    """pm_poisson_force / _vjp with PM_FLAG_GRAD_REAL (potential spectrum, ONE C2R, Table 2 stencil in real space;
+    transposed: stencil divergence, ONE R2C) against the UNCHANGED oracle with the Fourier-space symbols."""
+    box = 100.0
+    interlace = 1 if (m == 64 and grad_order == 4) else 0
+    d = gen.random_mesh(m, 500 + m, 2)
+    flags = pm.FLAG_GRAD_REAL | (0 if fused else pm.FLAG_NO_XFUSE)
+    ctx = pm.pm_create(pm.PMParams(m=m, box=box, max_particles=8, worder=3, grad_order=grad_order, lap_order=0,
+                                   deconv_pow=2, coeff=0.9, interlace=interlace, flags=flags))
+    g = [torch.empty(m, m, m, device="cuda") for _ in range(3)]
+    d2 = dev(d[1]) if interlace else None
+    pm.pm_poisson_force(ctx, dev(d[0]), g, delta_mesh2=d2)
+    ref = po.poisson_force(d[0], box, 3, grad_order, 0, 2, coeff=0.9, delta_mesh2=d[1] if interlace else None)
+    for a in range(3):
+        check(f"fwd/g{a}", g[a], ref[a], 3e-6)
+    cot = gen.random_mesh(m, 600 + m, 3)
+    c1 = torch.empty(m, m, m, device="cuda")
+    c2 = torch.empty(m, m, m, device="cuda") if interlace else None
+    pm.pm_poisson_force_vjp(ctx, [dev(cot[a]) for a in range(3)], c1, delta_cot2=c2)
+    r = po.poisson_force_vjp([cot[a] for a in range(3)], box, 3, grad_order, 0, 2, coeff=0.9, interlace=bool(interlace))
+    if interlace:
+        check("tr/c1", c1, r[0], 3e-6)
+        check("tr/c2", c2, r[1], 3e-6)
+    else:
+        check("tr/c1", c1, r, 3e-6)
+    pm.pm_destroy(ctx)
+
+
+@pytest.mark.parametrize("name,n_p,interlace", [("headline", 64, 0), ("cfg1", 64, 1), ("cfg1", 48, 2), ("cfg2", 64, 0)])
+def test_real_gradient_force_and_vjp(pm, name, n_p, interlace):
+    pos, c = gen.make_config_positions(name, n_p=n_p)
+    c = dict(c, interlace=interlace)
+    n = pos.shape[0]
+    lam = gen.gaussian_cotangent(n, 2100)
+    ctx = pm.pm_create(params_of(pm, c, n, flags=pm.FLAG_GRAD_REAL))
+    f, xb = torch.empty(n, 3, device="cuda"), torch.empty(n, 3, device="cuda")
+    pm.pm_force(ctx, dev(pos), f)
+    pm.pm_force_vjp(ctx, dev(pos), dev(lam), xb)
+    pm.pm_destroy(ctx)
+    check("force", f, po.force(pos, c["m"], c["box"], **oracle_kw(c)), 1e-5)
+    check("vjp", xb, po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c)), 1e-5)
+
+
+def test_real_gradient_headline_full_size_sampled(pm):
+    """The one-C2R variant on the bench workload at full size (same sampled comparison as the reference path)."""
+    from test_gpu_fullsize import sampled_force_and_vjp, uniform_sample
+
+    old = po.FFT_WORKERS
+    po.FFT_WORKERS = -1
+    try:
+        sampled_force_and_vjp(pm, "headline", uniform_sample, with_vjp=True, flags=pm.FLAG_GRAD_REAL)
+    finally:
+        po.FFT_WORKERS = old
+
+
+# ---- NEXT-3: ES kernel-gradient force ----------------------------------------------------------------------------
+@pytest.mark.parametrize("sigma,eps,width", [(2.0, 1e-6, 0), (2.0, 1e-4, 0), (1.25, 0.5, 5), (2.0, 1e-6, 8)])
+def test_kernel_gradient_force(pm, sigma, eps, width):
+    pos, c = gen.make_config_positions("cfg3", n_p=48)
+    n = pos.shape[0]
+    ctx = pm.pm_create(pm.PMParams(m=c["m"], box=c["box"], max_particles=n, method=1, nufft_sigma=sigma, nufft_eps=eps,
+                                   nufft_width=width, grad_order=0, lap_order=0, flags=pm.FLAG_KERNEL_GRAD))
+    f = torch.empty(n, 3, device="cuda")
+    pm.pm_force(ctx, dev(pos), f)
+    with pytest.raises(pm.PMError):
+        pm.pm_force_vjp(ctx, dev(pos), dev(pos), f)  # not built: needs second derivatives of the kernel
+    pm.pm_destroy(ctx)
+    ref = no.nufft_force(pos, c["m"], c["box"], sigma=sigma, eps=eps, width=width, kernel_grad=True)
+    w, beta = no.es_params(eps, sigma, width)
+    # The derivative of the ES kernel, ~ beta e^-beta / sqrt(1 - z^2) near the support edge, is unbounded there (R13):
+    # a particle within ~1e-6 of an edge carries an O(1) error in that one weight.  At w >= 7 (e^-beta <= 1e-7) this
+    # is invisible; at the narrow widths it is what the GPU-vs-oracle difference consists of (measured 1.5e-5 at
+    # w = 5, sigma = 2).  The bar is north_star's 10 x the tolerance the width stands for, eps_w = 10^-(w-1).
+    tol = max(1e-5, 10.0 * 10.0 ** (-(w - 1)))
+    check("force", f, ref, tol, maxabs_tol=max(1e-4, 30.0 * tol))
+
+
+def test_kernel_gradient_vs_bruteforce_definition(pm):
+    m, box = 12, 30.0
+    pos = gen.uniform_random(700, box, 63)
+    ctx = pm.pm_create(pm.PMParams(m=m, box=box, max_particles=700, method=1, nufft_sigma=2.0, nufft_eps=1e-6,
+                                   grad_order=0, lap_order=0, flags=pm.FLAG_KERNEL_GRAD))
+    f = torch.empty(700, 3, device="cuda")
+    pm.pm_force(ctx, dev(pos), f)
+    pm.pm_destroy(ctx)
+    check("vs_nudft", f, no.nudft_force_bruteforce(pos, m, box), 1e-5)  # 10 eps, eps = 1e-6
+
+
+# ---- NEXT-2: forward-mode rules ------------------------------------------------------------------------------------
+M, BOX = 40, 100.0
+
+
+def mixed_positions(n, box, seed, clump=True):
+    rng = np.random.default_rng(seed)
+    a = gen.uniform_random(n, box, seed)
+    cl = (rng.random((5000 if clump else 0, 3)) * 0.02 + 0.31) * box
+    edge = np.array([[0.0, 0.0, 0.0], [box * (1 - 2e-7), box * 0.5, 0.0], [-0.25 * box, 1.5 * box, 2.125 * box]])
+    return np.concatenate([a, cl, edge]).astype(np.float32)
+
+
+@pytest.mark.parametrize("worder", [2, 3, 4])
+@pytest.mark.parametrize("shifted", [False, True])
+@pytest.mark.parametrize("clump", [False, True])
+def test_assign_jvp_parity(pm, worder, shifted, clump):
+    """Tangent of the scatter, Eq. C.13a.  The deposits of one particle sum to zero (sum_j dW_j = 0), so the result
+    is a cancelling sum; the 32-bit fixed-point accumulator's quantum is 2^-30 of the work item's bound
+    sum_i (|w~_i| + |w_i| |X~_i|_1 / Delta).  Without a clump (items of a few hundred particles) that is fp32-like
+    (bar 2e-6); with 5000 particles inside one cell (one item of 4096 with ~1e4 of summed |deposits| against node
+    sums of ~20) the error is the quantisation noise of that item, measured 0.7e-5 .. 1.7e-5 of the mesh norm."""
+    pos = mixed_positions(20000, BOX, 111 + worder, clump)
+    tol = 3e-5 if clump else 2e-6
+    n = pos.shape[0]
+    rng = np.random.default_rng(112)
+    w = rng.standard_normal(n).astype(np.float32)
+    tX = rng.standard_normal((n, 3)).astype(np.float32)
+    tw = rng.standard_normal(n).astype(np.float32)
+    pre = gen.random_mesh(M, 113)[0]
+    shift = (0.5 * BOX / M,) * 3 if shifted else None
+    ctx = pm.pm_create(pm.PMParams(m=M, box=BOX, max_particles=n, worder=worder))
+    mt = dev(pre)
+    pm.pm_assign_jvp(ctx, dev(pos), dev(w), mt, pos_tan=dev(tX), w_tan=dev(tw), shift=shift)
+    ref = po.scatter_jvp(pos, M, BOX, worder, weights=w, pos_tan=tX, w_tan=tw, shift=shift, mesh_tan=pre)
+    check("both", mt, ref, tol, maxabs_tol=MAXABS_SIGNED_SCATTER)
+    mt2 = torch.zeros(M, M, M, device="cuda")   # unit weights, positions only
+    pm.pm_assign_jvp(ctx, dev(pos), None, mt2, pos_tan=dev(tX), shift=shift)
+    check("pos_only", mt2, po.scatter_jvp(pos, M, BOX, worder, pos_tan=tX, shift=shift), tol,
+          maxabs_tol=2 * MAXABS_SIGNED_SCATTER)
+    pm.pm_destroy(ctx)
+
+
+@pytest.mark.parametrize("worder", [2, 3, 4])
+@pytest.mark.parametrize("ncomp", [1, 3])
+@pytest.mark.parametrize("with_mesh_tan", [False, True])
+def test_interp_jvp_parity(pm, worder, ncomp, with_mesh_tan):
+    pos = mixed_positions(20000, BOX, 121 + worder)
+    n = pos.shape[0]
+    tX = np.random.default_rng(122).standard_normal((n, 3)).astype(np.float32)
+    meshes = gen.random_mesh(M, 123, ncomp)
+    tm = gen.random_mesh(M, 124, ncomp) if with_mesh_tan else None
+    shift = (0.5 * BOX / M, 0.0, -1.25 * BOX / M) if worder == 3 else None
+    ctx = pm.pm_create(pm.PMParams(m=M, box=BOX, max_particles=n, worder=worder))
+    out = torch.empty(n, ncomp, device="cuda")
+    pm.pm_interp_jvp(ctx, [dev(meshes[a]) for a in range(ncomp)], dev(pos), out, pos_tan=dev(tX),
+                     mesh_tan=[dev(tm[a]) for a in range(ncomp)] if with_mesh_tan else None, shift=shift)
+    ref = np.stack([po.gather_jvp(meshes[a], pos, BOX, worder, pos_tan=tX, mesh_tan=tm[a] if with_mesh_tan else None,
+                                  shift=shift) for a in range(ncomp)], axis=1)
+    check("out_tan", out, ref, 2e-6)
+    pm.pm_destroy(ctx)
+
+
+def test_jvp_vjp_duality_on_gpu(pm):
+    """<JVP(t), c> = <t, VJP(c)> with the GPU operators (rule table :949-960)."""
+    pos = mixed_positions(20000, BOX, 131)
+    n = pos.shape[0]
+    rng = np.random.default_rng(132)
+    w = rng.standard_normal(n).astype(np.float32)
+    tX, tw = rng.standard_normal((n, 3)).astype(np.float32), rng.standard_normal(n).astype(np.float32)
+    cm = gen.random_mesh(M, 133)[0]
+    for worder in (2, 3, 4):
+        ctx = pm.pm_create(pm.PMParams(m=M, box=BOX, max_particles=n, worder=worder))
+        mt = torch.zeros(M, M, M, device="cuda")
+        pm.pm_assign_jvp(ctx, dev(pos), dev(w), mt, pos_tan=dev(tX), w_tan=dev(tw))
+        pc, wc = torch.empty(n, 3, device="cuda"), torch.empty(n, device="cuda")
+        pm.pm_assign_vjp(ctx, dev(pos), dev(w), dev(cm), pos_cot=pc, w_cot=wc)
+        lhs = float((mt.double() * dev(cm).double()).sum())
+        rhs = float((pc.double() * dev(tX).double()).sum() + (wc.double() * dev(tw).double()).sum())
+        scale = float(mt.double().norm() * dev(cm).double().norm())  # Cauchy-Schwarz scale of the pairing
+        record_error(f"jvp_vjp_duality/worder={worder}", abs(lhs - rhs) / scale, 1e-6)
+        assert abs(lhs - rhs) <= 1e-6 * scale
+        pm.pm_destroy(ctx)
+
+
+# ---- NEXT-1: DKD step and its adjoint ----------------------------------------------------------------------------------
+def dkd_setup(name, n_p, seed):
+    pos, c = gen.make_config_positions(name, n_p=n_p)
+    n = pos.shape[0]
+    rng = np.random.default_rng(seed)
+    vel = (rng.standard_normal((n, 3)) * 0.4 * c["box"] / c["m"]).astype(np.float32)
+    return pos, vel, c, n
+
+
+COEFS = [(0.6, 0.4, 0.93, 0.21), (0.5, 0.5, 1.04, 0.17)]
+
+
+@pytest.mark.parametrize("name,n_p,interlace", [("cfg1", 48, 1), ("cfg1", 48, 2), ("headline", 64, 0), ("cfg4", 48, 0)])
+def test_dkd_step_parity(pm, name, n_p, interlace):
+    """Two forward steps (Eq. 2.14) against the oracle with the fp32 state arithmetic of reading R18: errors are
+    measured on what a step changes, dX (minimum image) and V."""
+    pos, vel, c, n = dkd_setup(name, n_p, 140)
+    c = dict(c, interlace=interlace, coeff=0.7)
+    box = c["box"]
+    ctx = pm.pm_create(params_of(pm, c, n, coeff=0.7))
+    X, V = dev(pos), dev(vel)
+    kw = oracle_kw(c, coeff=0.7)
+    acc = lambda x: po.force(x, c["m"], box, **kw)  # noqa: E731
+    Xo, Vo = pos, vel
+    for s, cf in enumerate(COEFS):
+        X0 = Xo
+        pm.pm_dkd_step(ctx, X, V, *cf)
+        Xo, Vo = dk.dkd_step(Xo, Vo, *cf, acc, box, state_dtype=np.float32)
+        check(f"step{s}/V", V, Vo, 1e-5)
+        check(f"step{s}/dX", minimg(X.cpu().numpy().astype(np.float64) - X0, box), minimg(Xo.astype(np.float64) - X0, box), 1e-5)
+        assert float(X.min()) >= 0.0 and float(X.max()) < box
+    pm.pm_destroy(ctx)
+
+
+@pytest.mark.parametrize("name,n_p,interlace,flags", [("cfg1", 48, 1, 0), ("cfg1", 32, 2, 0), ("headline", 64, 0, 0),
+                                                       ("headline", 64, 0, 4)])
+def test_dkd_adjoint_step_parity(pm, name, n_p, interlace, flags):
+    """Two forward steps, then the two backward-in-time steps of Table 3 with seeded cotangents: (X, V, X*, V*) and
+    the scalar adjoints (tau1*, tau2*, alpha*, beta*) of each step against the oracle."""
+    pos, vel, c, n = dkd_setup(name, n_p, 150)
+    c = dict(c, interlace=interlace, coeff=0.7)
+    box = c["box"]
+    kw = oracle_kw(c, coeff=0.7)
+    acc = lambda x: po.force(x, c["m"], box, **kw)  # noqa: E731
+    vjp = lambda x, lam: po.force_vjp(x, lam, c["m"], box, **kw)  # noqa: E731
+    ctx = pm.pm_create(params_of(pm, c, n, coeff=0.7, flags=flags))
+    X, V = dev(pos), dev(vel)
+    Xo, Vo = pos, vel
+    for cf in COEFS:
+        pm.pm_dkd_step(ctx, X, V, *cf)
+        Xo, Vo = dk.dkd_step(Xo, Vo, *cf, acc, box, state_dtype=np.float32)
+    # start the backward pass of BOTH sides from the oracle's final state, so that each step is compared on its own
+    X, V = dev(Xo), dev(Vo)
+    rng = np.random.default_rng(151)
+    Xs0 = rng.standard_normal((n, 3)).astype(np.float32)
+    Vs0 = rng.standard_normal((n, 3)).astype(np.float32)
+    Xs, Vs = dev(Xs0), dev(Vs0)
+    Xso, Vso = Xs0, Vs0
+    sadj = torch.zeros(4, dtype=torch.float64, device="cuda")
+    for s, cf in enumerate(reversed(COEFS)):
+        X1 = Xo
+        pm.pm_dkd_step_adjoint(ctx, X, V, Xs, Vs, *cf, scalar_adj=sadj)
+        Xo, Vo, Xso, Vso, adj = dk.dkd_step_adjoint(Xo, Vo, Xso, Vso, *cf, acc, vjp, box, state_dtype=np.float32)
+        check(f"back{s}/V", V, Vo, 1e-5)
+        check(f"back{s}/dX", minimg(X.cpu().numpy().astype(np.float64) - X1, box), minimg(Xo.astype(np.float64) - X1, box), 1e-5)
+        check(f"back{s}/Xs", Xs, Xso, 1e-5)
+        check(f"back{s}/Vs", Vs, Vso, 1e-5)
+        got = sadj.cpu().numpy()
+        for k, nm in enumerate(("tau1", "tau2", "alpha", "beta")):
+            scale = np.sqrt(n) * 3.0  # the dot products are sums of 3N products of O(1) numbers
+            record_error(f"dkd_adjoint/{name}/back{s}/{nm}", abs(got[k] - adj[nm]) / scale, 1e-5)
+            assert abs(got[k] - adj[nm]) <= 1e-5 * max(scale, abs(adj[nm])), (nm, got[k], adj[nm])
+    # time reversibility: the primal state is back at the start to fp32 rounding of the positions
+    d = minimg(X.cpu().numpy().astype(np.float64) - pos, box)
+    assert np.abs(d).max() <= 5e-4 * box / c["m"]
+    pm.pm_destroy(ctx)
+
+
+def test_force_vjp_reuses_pinned_meshes(pm):
+    """pm_bin + pm_force + pm_force_vjp on the same pinned positions: the VJP reuses the force meshes; the result
+    must equal the call that recomputes them."""
+    pos, c = gen.make_config_positions("cfg1", n_p=48)
+    n = pos.shape[0]
+    lam = gen.gaussian_cotangent(n, 2200)
+    ctx = pm.pm_create(params_of(pm, c, n))
+    dp, dl = dev(pos), dev(lam)
+    a = torch.empty(n, 3, device="cuda")
+    pm.pm_force_vjp(ctx, dp, dl, a)  # recomputes
+    pm.pm_bin(ctx, dp)
+    f = torch.empty(n, 3, device="cuda")
+    pm.pm_force(ctx, dp, f)
+    pm.pm_set_profiling(ctx, True)
+    b = torch.empty(n, 3, device="cuda")
+    pm.pm_force_vjp(ctx, dp, dl, b)
+    ms, _ = pm.pm_get_stage_ms(ctx)
+    assert ms["assign"] == 0.0 and ms["fft_fwd"] == 0.0 and ms["vjp_gather"] > 0.0  # forward part skipped
+    check("reuse_vs_recompute", b, a.cpu().numpy(), 2e-6)
+    check("vs_oracle", b, po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c)), 1e-5)
+    pm.pm_destroy(ctx)
+
+
+# ---- NEXT-4: power spectrum, sheet resampling -------------------------------------------------------------------------
+@pytest.mark.parametrize("worder,interlace,deconvolve", [(2, 0, True), (3, 1, True), (4, 1, False), (2, 1, True)])
+def test_power_spectrum_parity(pm, worder, interlace, deconvolve):
+    pos, c = gen.make_config_positions("cfg1", n_p=64)
+    n = pos.shape[0]
+    m, box, nbins = c["m"], c["box"], 40
+    ctx = pm.pm_create(pm.PMParams(m=m, box=box, max_particles=n, worder=worder, interlace=interlace))
+    k, P, cnt = (torch.zeros(nbins, dtype=torch.float64, device="cuda") for _ in range(3))
+    pm.pm_power_spectrum(ctx, dev(pos), k, P, cnt, deconvolve=deconvolve)
+    ko, Po, co = ao.power_spectrum(pos, m, box, nbins, worder=worder, interlace=interlace, deconvolve=deconvolve)
+    assert np.array_equal(cnt.cpu().numpy(), co)  # mode counts: integer work, exact
+    assert np.abs(k.cpu().numpy() - ko).max() <= 1e-12 * ko.max()
+    check("P", P, Po, 1e-5, maxabs_tol=1e-3)
+    # cross spectrum with a translated copy
+    pos2 = pos.copy()
+    pos2[:, 0] = np.mod(pos2[:, 0] + np.float32(3.0 * box / m), np.float32(box))
+    pm.pm_power_spectrum(ctx, dev(pos), k, P, cnt, pos2=dev(pos2), deconvolve=deconvolve)
+    _, Pc, _ = ao.power_spectrum(pos, m, box, nbins, worder=worder, interlace=interlace, deconvolve=deconvolve, pos2=pos2)
+    check("Pcross", P, Pc, 2e-5, maxabs_tol=1e-3)
+    pm.pm_destroy(ctx)
+
+
+@pytest.mark.parametrize("n_p,r", [(16, 2), (24, 3), (32, 1)])
+def test_sheet_resample_parity(pm, n_p, r):
+    box, m = 200.0, 32
+    pos = gen.lattice_displaced(n_p, m, box, 1.5, 160 + n_p)
+    ctx = pm.pm_create(pm.PMParams(m=m, box=box, max_particles=8))
+    out = torch.empty((n_p * r) ** 3, 3, device="cuda")
+    pm.pm_sheet_resample(ctx, dev(pos), n_p, r, out)
+    ref = ao.sheet_resample(pos, n_p, box, r)
+    d = minimg(out.cpu().numpy().astype(np.float64) - ref, box)
+    record_error(f"sheet_resample/n_p={n_p}/r={r}", float(np.abs(d).max() / box), 1e-7)
+    assert np.abs(d).max() <= 1e-7 * box  # fp32 rounding of the stored positions (ulp(L)/2 = 3e-8 L)
+    o = out.cpu().numpy()
+    assert o.min() >= 0.0 and o.max() < box
+    pm.pm_destroy(ctx)

@@ -14,7 +14,7 @@ torch = pytest.importorskip("torch")
 from oracle import pm_oracle as po
 from pm_inputs import generators as gen
 
-from parity_util import check, record_error, rel_l2
+from parity_util import MAXABS_SIGNED_SCATTER, check, record_error, rel_l2
 
 pytestmark = pytest.mark.gpu
 
@@ -122,7 +122,7 @@ def test_interp_vjp_parity(pm, worder, ncomp):
         # random-sign weights in a dense clump: the node sums cancel, while the fixed-point quantum is 2^-30 of the
         # work item's bound sum|w| * Wmax^3 ("Parity bars"); with items of up to 4096 particles that is
         # the accuracy of an fp32 accumulation in the same order, not better
-        check("mesh_cot[a]", mesh_cot[a], ref, 5e-6)
+        check("mesh_cot[a]", mesh_cot[a], ref, 5e-6, maxabs_tol=MAXABS_SIGNED_SCATTER)
     ref_p = np.zeros((n, 3))
     for a in range(ncomp):
         for b in range(3):
@@ -296,7 +296,8 @@ def test_pm_bin_pinned_records_are_reused(pm):
         pm.pm_interp_vjp(ctx, d_m, d_pos, dev(cot), mesh_cot=mc, pos_cot=pc)
         refp = np.zeros((n, 3))
         for a in range(3):
-            check(f"pinned/mesh_cot{a}", mc[a], po.scatter(pos, M, BOX, worder, weights=cot[:, a]), 5e-6)
+            check(f"pinned/mesh_cot{a}", mc[a], po.scatter(pos, M, BOX, worder, weights=cot[:, a]), 5e-6,
+                  maxabs_tol=MAXABS_SIGNED_SCATTER)
             for b in range(3):
                 refp[:, b] += cot[:, a] * po.gather(meshes[a], pos, BOX, worder, deriv_axis=b)
         check("pinned/pos_cot", pc, refp, 2e-6)

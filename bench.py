@@ -31,9 +31,12 @@ UNIT = "particles/s"
 
 
 # ---------------------------------------------------------------------------------------------------------
-def algorithmic_bytes(n: int, g: int) -> dict:
+NOMINAL_HBM_GBS = 8000.0  # north_star: "B200's ~8 TB/s peak"
+
+
+def algorithmic_bytes(n: int, g: int, grad_real: bool = False) -> dict:
     """SURVEY 8(d) / DESIGN.md "Algorithmic bytes": what the method itself must move (fp32), per stage."""
-    return {
+    ab = {
         "bin": 12 * n + 16 * n,            # the build's own step: one read of the positions + the records written
                                            # (single-pass bucketed sort; its zero-fill of the mesh is not counted)
         "assign": 12 * n + 4 * g,          # positions in, mesh written once
@@ -41,7 +44,16 @@ def algorithmic_bytes(n: int, g: int) -> dict:
         "kspace": 4 * g + 12 * g,
         "fft_inv": 24 * g,
         "interp": 12 * n + 12 * g + 12 * n,  # positions + 3 meshes in, forces out
+        # reverse mode (SURVEY 8(d) "force-VJP extra")
+        "vjp_scatter": 24 * n + 12 * g,    # positions + cotangents in, 3 meshes out
+        "vjp_kspace": 24 * g + 16 * g + 8 * g,  # 3 R2C floors, transposed kernel 12G in + 4G out, 1 C2R floor
+        "vjp_gather": 36 * n + 16 * g,     # positions, cotangents, position cotangents out; 4 meshes in
+        # DKD elementwise pass: X, V read, X written
+        "step": 36 * n,
     }
+    if grad_real:  # PM_FLAG_GRAD_REAL: potential only through Fourier space, stencil in real space
+        ab.update(kspace=4 * g + 4 * g, fft_inv=8 * g, gradient=4 * g + 12 * g)  # (the VJP stays in Fourier space)
+    return ab
 
 
 class ClockSampler:
@@ -96,16 +108,23 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_sample_run(cfg_name: str, n_p: int):
-    """One oracle force evaluation of the same configuration at reduced size; returns (seconds, particles)."""
+def oracle_sample_run(cfg_name: str, n_p: int, fft_workers: int = 1):
+    """One oracle force evaluation of the same configuration at reduced size; returns (seconds, particles).
+    fft_workers != 1 runs the oracle's FFT library step on that many host threads (-1: all); its scatter / gather
+    loops are single-threaded NumPy by construction."""
     from oracle import pm_oracle as po
     from pm_inputs import generators as gen
 
     pos, c = gen.make_config_positions(cfg_name, n_p=n_p)
-    t0 = time.perf_counter()
-    po.force(pos, c["m"], c["box"], worder=c["worder"], interlace=c["interlace"], grad_order=c["grad_order"],
-             lap_order=c["lap_order"], deconv_pow=c["deconv_pow"])
-    return time.perf_counter() - t0, pos.shape[0]
+    old = po.FFT_WORKERS
+    po.FFT_WORKERS = fft_workers
+    try:
+        t0 = time.perf_counter()
+        po.force(pos, c["m"], c["box"], worder=c["worder"], interlace=c["interlace"], grad_order=c["grad_order"],
+                 lap_order=c["lap_order"], deconv_pow=c["deconv_pow"])
+        return time.perf_counter() - t0, pos.shape[0]
+    finally:
+        po.FFT_WORKERS = old
 
 
 def replica_seed(seed: int, rank: int) -> int:
@@ -167,6 +186,133 @@ def run_reference(args) -> int:
     return 0
 
 
+def csrc_fingerprint() -> str:
+    """Hash of the kernel sources: an ncu traffic figure is only quoted for the library it was measured on."""
+    import hashlib
+
+    h = hashlib.sha1()
+    d = os.path.join(ROOT, "paper_2510_05206_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def load_peak():
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        return float(json.load(open(peaks_path))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (burst copy)"
+    return 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
+
+
+def make_positions(gen, name, rank, n_p=0):
+    c = dict(gen.CONFIGS[name])
+    if n_p:
+        return gen.make_config_positions(name, n_p=n_p)
+    c["seed"] = replica_seed(c["seed"], rank)
+    if c.get("clustered"):
+        pos = gen.clustered_halos(c["n_p"] ** 3, c["m"], c["box"], c["seed"],
+                                  lattice_shape=(c["n_p"], c["n_p"], c["n_p"] // 2), rms_cells=c["rms"])
+    else:
+        pos = gen.lattice_displaced(c["n_p"], c["m"], c["box"], c["rms"], c["seed"])
+    return pos, c
+
+
+def params_for(pm, c, n, flags=0):
+    return pm.PMParams(m=c["m"], box=c["box"], max_particles=n, worder=c.get("worder", 2),
+                       interlace=c.get("interlace", 0), deconv_pow=c.get("deconv_pow", 2),
+                       grad_order=c.get("grad_order", 0), lap_order=c.get("lap_order", 0),
+                       method=1 if c.get("nufft") else 0, nufft_sigma=c.get("sigma", 2.0),
+                       nufft_eps=c.get("eps", 1e-6), nufft_width=c.get("width", 0), flags=flags)
+
+
+def stage_table(stage_ms, ab, peak, names):
+    out = {}
+    for k in names:
+        if stage_ms.get(k, 0.0) > 0 and k in ab:
+            gbs = ab[k] / (stage_ms[k] * 1e-3) / 1e9
+            out[k] = {"ms": round(stage_ms[k], 4), "alg_GB": round(ab[k] / 1e9, 4), "GBps": round(gbs, 1),
+                      "frac": round(gbs / peak, 4), "frac_nominal_8TBps": round(gbs / NOMINAL_HBM_GBS, 4)}
+        elif stage_ms.get(k, 0.0) > 0:
+            out[k] = {"ms": round(stage_ms[k], 4)}
+    return out
+
+
+FORCE_STAGES = ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "gradient", "interp")
+VJP_STAGES = FORCE_STAGES[:-1] + ("vjp_scatter", "vjp_kspace", "vjp_gather")
+
+
+def time_call(torch, fn, steps, warmup, barrier=None):
+    """ms per call: `steps` calls between two CUDA events on the current stream (the stream the library launches on)."""
+    for _ in range(warmup):
+        fn()
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
+def profile_stages(pm, ctx, fn, steps):
+    """Per-stage CUDA-event durations from a separate pass (events are only recorded here, never in a timed loop)."""
+    pm.pm_set_profiling(ctx, True)
+    acc = {k: 0.0 for k in pm.STAGE_NAMES}
+    launches = 0
+    for _ in range(steps):
+        fn()
+        ms, launches = pm.pm_get_stage_ms(ctx)
+        for k in acc:
+            acc[k] += ms[k] / steps
+    pm.pm_set_profiling(ctx, False)
+    return acc, launches
+
+
+def run_config(torch, pm, gen, name, rank, local, peak, steps, warmup, with_vjp, flags=0, n_p=0, pos_c=None):
+    """Force (and VJP) throughput and stage times of one named configuration; its own clock sample."""
+    pos_np, c = pos_c if pos_c is not None else make_positions(gen, name, rank, n_p)
+    n = pos_np.shape[0]
+    ctx = pm.pm_create(params_for(pm, c, n, flags))
+    g = ctx.G  # mesh the FFTs and the scatter / gather run on (NUFFT: the fine grid)
+    pos = torch.from_numpy(pos_np).cuda()
+    out = torch.empty(n, 3, device="cuda")
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms = time_call(torch, lambda: pm.pm_force(ctx, pos, out), steps, warmup)
+    st, launches = profile_stages(pm, ctx, lambda: pm.pm_force(ctx, pos, out), max(2, steps // 2))
+    ab = algorithmic_bytes(n, g, bool(flags & pm.FLAG_GRAD_REAL))
+    res = {"workload": f"{name}: N={c['n_p']}^3, mesh {c['m']}^3" + (", NUFFT fine grid %d^3 w=%d" % (ctx.mg, ctx.nufft_width) if c.get("nufft") else ""),
+           "particles": n, "ms_per_step": round(ms, 4), "particles_per_s": n / (ms * 1e-3), "launches_per_step": launches,
+           "stages": stage_table(st, ab, peak, FORCE_STAGES)}
+    if c.get("nufft"):  # spreading / interpolation against the measured shared-memory ceilings, not HBM
+        w3 = ctx.nufft_width ** 3
+        atom, lds = pm.pm_smem_peak(ctx, 1), pm.pm_smem_peak(ctx, 0)
+        res["smem_ceiling"] = {"atomics_per_s": atom, "loads_per_s": lds, "how": "pm_smem_peak: conflict-free micro-kernel"}
+        for k, ops, ceil in (("assign", w3 * n, atom), ("interp", 3 * w3 * n, lds)):
+            if k in res["stages"]:
+                res["stages"][k].update(bound="smem", lane_ops_per_s=ops / (st[k] * 1e-3), frac_smem=round(ops / (st[k] * 1e-3) / ceil, 4))
+    if with_vjp:
+        lam = torch.from_numpy(gen.gaussian_cotangent(n, c.get("cot_seed", 2000))).cuda()
+        ms_v = time_call(torch, lambda: pm.pm_force_vjp(ctx, pos, lam, out), max(2, steps // 2), 2)
+        stv, _ = profile_stages(pm, ctx, lambda: pm.pm_force_vjp(ctx, pos, lam, out), 2)
+        res["vjp"] = {"ms_per_call": round(ms_v, 4), "stages": stage_table(stv, ab, peak, VJP_STAGES)}
+        del lam
+    res["clocks"] = sampler.stop()
+    pm.pm_destroy(ctx)
+    del pos, out
+    torch.cuda.empty_cache()
+    return res
+
+
 def run_ours(args) -> int:
     import torch
     import torch.distributed as dist
@@ -182,26 +328,13 @@ def run_ours(args) -> int:
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peak, peak_src = load_peak()
 
     # ---- workload: one independent replica per rank (replicas only, no collective) ----------
-    c = dict(gen.CONFIGS[args.config])
-    if args.n_p:
-        pos_np, c = gen.make_config_positions(args.config, n_p=args.n_p)
-    else:
-        c["seed"] = replica_seed(c["seed"], rank)
-        if c.get("clustered"):
-            pos_np = gen.clustered_halos(c["n_p"] ** 3, c["m"], c["box"], c["seed"],
-                                         lattice_shape=(c["n_p"], c["n_p"], c["n_p"] // 2), rms_cells=c["rms"])
-        else:
-            pos_np = gen.lattice_displaced(c["n_p"], c["m"], c["box"], c["rms"], c["seed"])
+    pos_np, c = make_positions(gen, args.config, rank, args.n_p)
     n = pos_np.shape[0]
     g = c["m"] ** 3
-    params = pm.PMParams(m=c["m"], box=c["box"], max_particles=n, worder=c.get("worder", 2),
-                         interlace=c.get("interlace", 0), deconv_pow=c.get("deconv_pow", 2),
-                         grad_order=c.get("grad_order", 0), lap_order=c.get("lap_order", 0),
-                         method=1 if c.get("nufft") else 0, nufft_sigma=c.get("sigma", 2.0),
-                         nufft_eps=c.get("eps", 1e-6))
-    ctx = pm.pm_create(params)
+    ctx = pm.pm_create(params_for(pm, c, n))
     pos_host = torch.from_numpy(pos_np).pin_memory()
     force_host = torch.empty(n, 3, dtype=torch.float32).pin_memory()
     pos = pos_host.cuda()
@@ -212,34 +345,18 @@ def run_ours(args) -> int:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing ---------------------------------------------------------------------------
-    pm.pm_set_profiling(ctx, True)
+    # ---- device-resident timing (no events inside the library during the timed loop) ------------------------
+    pm.pm_set_profiling(ctx, False)
     for _ in range(args.warmup):
         pm.pm_force(ctx, pos, force)
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    stage_acc = {k: 0.0 for k in pm.STAGE_NAMES}
-    launches = 0
-    barrier()
-    e0.record()
-    for _ in range(args.steps):
-        pm.pm_force(ctx, pos, force)
-    e1.record()
-    barrier()
-    ms_total = e0.elapsed_time(e1)
-    # per-stage durations: a separate profiled pass (pm_get_stage_ms synchronises, so not inside the timed loop)
-    for _ in range(args.steps):
-        pm.pm_force(ctx, pos, force)
-        ms, nl = pm.pm_get_stage_ms(ctx)
-        launches = nl
-        for k in stage_acc:
-            stage_acc[k] += ms[k] / args.steps
+    ms_total = time_call(torch, lambda: pm.pm_force(ctx, pos, force), args.steps, 0, barrier) * args.steps
+    stage_acc, launches = profile_stages(pm, ctx, lambda: pm.pm_force(ctx, pos, force), args.steps)
     clocks = sampler.stop()
 
     # ---- end to end through the C ABI with HOST buffers (copies inside the timed region) -------------------
-    pm.pm_set_profiling(ctx, False)
     pm.pm_force_host(ctx, pos_host, force_host)  # warm-up (allocates the staging buffers)
     barrier()
     t0 = time.perf_counter()
@@ -251,6 +368,46 @@ def run_ours(args) -> int:
     checksum = float(force_host[:: max(1, n // 1000)].double().abs().sum())
 
     ms_total, e2e_ms = max_over_ranks([ms_total, e2e_s * 1e3], world, device="cuda")
+
+    # ---- beside the headline (rank 0 of a single-GPU run only; every block is a measurement of this run) ------
+    extras = {}
+    if rank == 0 and world == 1 and not args.headline_only and not c.get("nufft"):
+        lam = torch.from_numpy(gen.gaussian_cotangent(n, 2005)).cuda()
+        xbar = torch.empty(n, 3, device="cuda")
+        ab = algorithmic_bytes(n, g)
+        # reverse mode on the same workload
+        ms_v = time_call(torch, lambda: pm.pm_force_vjp(ctx, pos, lam, xbar), 5, 2)
+        stv, _ = profile_stages(pm, ctx, lambda: pm.pm_force_vjp(ctx, pos, lam, xbar), 3)
+        extras["vjp"] = {"call": "pm_force_vjp (forward meshes recomputed)", "ms_per_call": round(ms_v, 4),
+                         "stages": stage_table(stv, ab, peak, VJP_STAGES)}
+        pm.pm_bin(ctx, pos)
+        pm.pm_force(ctx, pos, force)
+        ms_r = time_call(torch, lambda: pm.pm_force_vjp(ctx, pos, lam, xbar), 5, 2)
+        extras["vjp"]["ms_per_call_reusing_pinned_force_meshes"] = round(ms_r, 4)
+        # one DKD step and one backward-in-time adjoint step on copies of the state
+        X, V = pos.clone(), (torch.randn(n, 3, device="cuda") * (0.3 * c["box"] / c["m"]))
+        Xs, Vs = lam.clone(), xbar.normal_()
+        coef = (0.5, 0.5, 0.97, 0.2)
+        ms_s = time_call(torch, lambda: pm.pm_dkd_step(ctx, X, V, *coef), 5, 2)
+        ms_a = time_call(torch, lambda: pm.pm_dkd_step_adjoint(ctx, X, V, Xs, Vs, *coef), 3, 1)
+        extras["dkd"] = {"step_ms": round(ms_s, 4), "adjoint_step_ms": round(ms_a, 4),
+                         "note": "Eq. 2.14 / Table 3 at the headline size; kick, second drift and the alpha*, beta* "
+                                 "reductions ride on the gather; the adjoint step shares one set of force meshes "
+                                 "between the primal kick-back and the VJP"}
+        del X, V, Xs, Vs, lam, xbar
+        pm.pm_destroy(ctx)
+        ctx = None
+        del pos, force
+        torch.cuda.empty_cache()
+        # the one-C2R variant (PM_FLAG_GRAD_REAL) on the same workload
+        extras["variants"] = {"grad_real": run_config(torch, pm, gen, args.config, rank, local, peak, args.steps,
+                                                      args.warmup, True, flags=pm.FLAG_GRAD_REAL, n_p=args.n_p,
+                                                      pos_c=(pos_np, c))}
+        if not args.no_other_configs and not args.n_p:
+            oc = {}
+            for name, vjp in (("cfg2", False), ("cfg4", True), ("cfg3", False)):
+                oc[name] = run_config(torch, pm, gen, name, rank, local, peak, 5, 3, vjp)
+            extras["other_configs"] = oc
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -260,41 +417,41 @@ def run_ours(args) -> int:
     e2e_value = whole_job_rate(world, n, e2e_steps, e2e_ms)
 
     # ---- roofline of the dominant hand-written kernel -----------------------------------------------------
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        peak = float(json.load(open(peaks_path))["hbm_gbs"])
-        peak_src = "MEASURED_PEAKS.json hbm_gbs (burst copy)"
-    else:
-        peak, peak_src = 6650.0, "fallback 6.65 TB/s (B200_PROFILING.md)"
     ab = algorithmic_bytes(n, g)
-    stages = {}
-    for k in ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "interp"):
-        if stage_acc[k] > 0:
-            gbs = ab[k] / (stage_acc[k] * 1e-3) / 1e9
-            stages[k] = {"ms": round(stage_acc[k], 4), "alg_GB": round(ab[k] / 1e9, 4), "GBps": round(gbs, 1),
-                         "frac": round(gbs / peak, 4)}
+    stages = stage_table(stage_acc, ab, peak, FORCE_STAGES)
     # the dominant hand-written KERNEL: stages that are one kernel launch each (assign = k_scatter_warp / k_scatter,
     # kspace = k_xfft_kspace / k_kspace_fwd, interp = k_gather); "bin" is six launches and is listed in `stages`
     own = {k: v for k, v in stages.items() if k in ("assign", "kspace", "interp")}
     dom = max(own, key=lambda k: own[k]["ms"])
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "dram_traffic.json")  # written from an ncu --set full capture
+    traffic, traffic_src = None, "none: no ncu capture of this configuration"
+    tp = os.path.join(ROOT, "profiles", "dram_traffic_r2.json")  # written from an ncu --set full capture
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(args.config, {}).get(dom)
+        tj = json.load(open(tp))
+        if tj.get("csrc_fingerprint") == csrc_fingerprint():
+            traffic = tj.get(args.config, {}).get(dom)
+            traffic_src = tj.get("source", "")
+        else:
+            traffic_src = "stale: the kernels changed since the ncu capture in profiles/ (" + tj.get("source", "") + ")"
     kernel_names = {"assign": "k_scatter_warp / k_scatter", "kspace": "k_xfft_kspace (x-FFTs + k-space) or k_kspace_fwd",
                     "interp": "k_gather"}
     roofline = {"bound": "hbm", "kernel": kernel_names[dom], "stage": dom, "achieved": stages[dom]["GBps"],
-                "peak": peak, "unit": "GB/s", "frac": stages[dom]["frac"], "traffic": traffic,
+                "peak": peak, "unit": "GB/s", "frac": stages[dom]["frac"],
+                "frac_nominal_8TBps": stages[dom]["frac_nominal_8TBps"], "traffic": traffic,
                 "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
-                "peak_source": peak_src}
+                "traffic_source": traffic_src, "peak_source": peak_src}
 
-    # ---- oracle timed beside it (bounded sample) ----------------------------------------------------------
+    # ---- oracle timed beside it (bounded samples; one core, and its FFT step on all cores) --------------------
     cpu = None
     if not args.no_cpu_baseline and not c.get("nufft"):
         dt, npart = oracle_sample_run(args.config, args.ref_np)
+        dta, _ = oracle_sample_run(args.config, args.ref_np, fft_workers=-1)
         cpu = {"value": npart / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"{args.config} at n_p={args.ref_np} (N={npart}), one evaluation, {dt:.1f} s; "
-                         f"NumPy fp64, single-threaded ({host_threads()} host threads available)"}
+               "sample": f"{args.config} at n_p={args.ref_np} (N={npart}), one evaluation, {dt:.1f} s; NumPy fp64, "
+                         f"single-threaded as it stands",
+               "all_cores": {"value": npart / dta, "cores": host_threads(), "seconds": round(dta, 2),
+                             "note": "same evaluation with the FFT library step on all host threads "
+                                     "(scipy.fft workers); the oracle's scatter / gather loops are single-threaded "
+                                     "NumPy by construction"}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -303,7 +460,7 @@ def run_ours(args) -> int:
         "config": {"workload": f"{args.config}: N={c['n_p']}^3 particles, mesh {c['m']}^3, box {c['box']}, "
                                f"worder={c.get('worder', 2)}, grad_order={c.get('grad_order', 0)}, "
                                f"deconv_pow={c.get('deconv_pow', 2)}, interlace={c.get('interlace', 0)}"
-                               + (", NUFFT" if c.get("nufft") else ""),
+                               + (", NUFFT" if c.get("nufft") else "") + "; reference path (three inverse FFTs)",
                    "particles": n, "mesh_cells": g, "replicas": world,
                    "l2_policy": "inputs larger than L2 (positions 1.6 GB, meshes 0.5 GB each); no flush",
                    "paper_context": "A100 40GB, JAX: 0.2 s/step at this setting (PAPER.md:552) = 6.7e8 particles/s"},
@@ -315,8 +472,10 @@ def run_ours(args) -> int:
         "stages": stages,
         "cpu_baseline": cpu,
     }
+    line.update(extras)
     print(json.dumps(line))
-    pm.pm_destroy(ctx)
+    if ctx is not None:
+        pm.pm_destroy(ctx)
     if world > 1:
         dist.destroy_process_group()
     return 0
@@ -333,6 +492,8 @@ def main(argv=None) -> int:
     ap.add_argument("--ref-np", dest="ref_np", type=int, default=0,
                     help="oracle sample size, particles per dim (default 192 beside our arm, 128 per reference step)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--headline-only", action="store_true", help="skip the VJP / DKD / variant / other-config blocks")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip cfg2 / cfg4 / cfg3 beside the headline")
     args = ap.parse_args(argv)
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3  # timing rule: at least 3 warm-up steps

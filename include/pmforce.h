@@ -68,7 +68,8 @@ typedef struct pm_params {
 #define PM_FLAG_NO_XFUSE 2    /* a2-a4: 3-D cuFFT + pointwise Fourier-space kernel instead of the fused x-FFT kernel */
 #define PM_FLAG_GRAD_REAL 4   /* a3-a4, method 0, grad_order 2/4/6: apply the gradient as the real-space stencil of
                                  Table 2 ("Real" column; its DFT IS the Fourier symbol) to the
-                                 potential mesh: ONE inverse FFT instead of three.  Same operator, other rounding. */
+                                 potential mesh: ONE inverse FFT instead of three.  Same operator, other rounding.
+                                 The transposed operator (VJP) keeps the Fourier-space form. */
 #define PM_FLAG_KERNEL_GRAD 8 /* method 1: force from the gradient of the ES kernel ("SPH-like"):
                                  the potential is interpolated with grad(phi_ES) instead of multiplying by i k.
                                  pm_force only (its VJP would need second derivatives of the kernel: PM_ESTATE). */
@@ -231,6 +232,11 @@ int pm_set_profiling(pm_ctx* ctx, int enable);
  * run) to ms_host[0..n-1], n <= PM_NUM_STAGES.  launches_host (or NULL) receives how many kernels of
  * this library (cuFFT's excluded) that call launched. */
 int pm_get_stage_ms(pm_ctx* ctx, float* ms_host, int n, int64_t* launches_host);
+/* Measured ceiling of the shared-memory pipe on this device, in lane operations per second (the roofline of the NUFFT
+ * spreading / interpolation kernels, which are bound by shared-memory atomics and loads, not by HBM):
+ * kind 0 = conflict-free 32-bit loads, 1 = conflict-free 32-bit integer atomic adds, 2 = 128-bit loads (counted as
+ * 4 words).  Runs a micro-kernel for a few milliseconds and synchronises. */
+int pm_smem_peak(pm_ctx* ctx, int kind, double* lane_ops_per_s_host, void* stream);
 
 #ifdef __cplusplus
 }

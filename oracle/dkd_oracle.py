@@ -10,9 +10,10 @@ Reading R18 -- precision of the state.  The paper's arrays are singl
 between operations exactly like the CUDA path does, with this arithmetic for a drift (every operation
 rounded to fp32, no fused multiply-add, so that both sides produce the same bits):
 
-    x' = x + (tau * v);   x' = x' - L * floor(x' / L);   x' < 0: x' += L;   x' >= L: x' -= L;   else 0
+    x' = x + (tau * v);   if x' < 0: x' = x' + L;   if x' >= L: x' = x' - L
 
-so the acceleration is evaluated at identical fp32 positions on both sides (a force evaluated at positions
+(a particle moves less than one box length per drift; a value that the addition rounds up to L is taken to 0 by
+the subtraction), so the acceleration is evaluated at identical fp32 positions on both sides (a force evaluated at positions
 that differ by one fp32 ulp of L differs by ~1e-5 relative).  Kicks and the adjoint
 updates are evaluated in fp64 from the fp32 state and rounded once.  ``state_dtype = numpy.float64`` keeps
 everything in fp64 and does not wrap (used by the pins: time reversibility, finite differences).
@@ -30,11 +31,9 @@ import numpy as np
 def wrap_fp32(x, box):
     """Periodic wrap of an fp32 array into [0, L) with fp32 operations only (see module docstring)."""
     L = np.float32(box)
-    x = np.asarray(x, dtype=np.float32)
-    y = x - L * np.floor(x / L)
+    y = np.asarray(x, dtype=np.float32)
     y = np.where(y < np.float32(0), y + L, y)
     y = np.where(y >= L, y - L, y)
-    y = np.where((y >= L) | (y < np.float32(0)), np.float32(0), y)
     return y.astype(np.float32)
 
 

@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = (
     "pm_interp", "pm_interp_vjp", "nufft_spread", "nufft_spread_vjp", "nufft_poisson_force",
     "nufft_poisson_force_vjp", "nufft_interp", "nufft_interp_vjp", "pm_force", "pm_force_vjp", "pm_force_host",
     "pm_set_profiling", "pm_get_stage_ms", "pm_assign_jvp", "pm_interp_jvp", "pm_dkd_step", "pm_dkd_step_adjoint",
-    "pm_power_spectrum", "pm_sheet_resample",
+    "pm_power_spectrum", "pm_sheet_resample", "pm_smem_peak",
 )
 
 STAGE_NAMES = ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "interp", "vjp_scatter", "vjp_kspace", "vjp_gather",
@@ -116,6 +116,7 @@ def load_library(build_if_missing: bool = False):
                                           vp, vp]),
         "pm_power_spectrum": (C.c_int, [vp, vp, i64, vp, i64, C.c_int, C.c_int, vp, vp, vp, vp]),
         "pm_sheet_resample": (C.c_int, [vp, vp, C.c_int32, C.c_int32, vp, vp]),
+        "pm_smem_peak": (C.c_int, [vp, C.c_int, C.POINTER(C.c_double), vp]),
         "pm_set_profiling": (C.c_int, [vp, C.c_int]),
         "pm_get_stage_ms": (C.c_int, [vp, C.POINTER(C.c_float), C.c_int, C.POINTER(i64)]),
     }
@@ -389,6 +390,13 @@ def pm_force_host(ctx, pos_host, force_host):
         raise ValueError("force_host must have 3*N elements")
     ctx.check(load_library().pm_force_host(ctx.handle, pos_host.data_ptr(), n, force_host.data_ptr(), _stream()),
               "pm_force_host")
+
+
+def pm_smem_peak(ctx, kind: int) -> float:
+    """Measured shared-memory lane operations per second (0 loads, 1 integer atomics, 2 128-bit loads)."""
+    v = C.c_double(0.0)
+    ctx.check(load_library().pm_smem_peak(ctx.handle, int(kind), C.byref(v), _stream()), "pm_smem_peak")
+    return float(v.value)
 
 
 def pm_set_profiling(ctx, enable: bool):

@@ -11,7 +11,11 @@ int es_gather_values_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
 template <int W>
 int es_gather_grad_w(Ctx* c, const GatherArgs& a, cudaStream_t st);
 
+#ifdef PMF_ES_WIDTHS  // development builds with fewer widths (build.py --es-widths): -D"PMF_ES_WIDTHS(X)=X(7)"
+#define ES_WIDTHS(X) PMF_ES_WIDTHS(X)
+#else
 #define ES_WIDTHS(X) X(4) X(5) X(6) X(7) X(8)
+#endif
 #define DECL(W)                                                                                    \
   template <>                                                                                      \
   int es_scatter_w<W>(Ctx*, int, const float*, int, float* const[], cudaStream_t);                 \

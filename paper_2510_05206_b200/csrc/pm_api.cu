@@ -163,7 +163,9 @@ int bin_for_path(Ctx* c, const float* pos, int64_t N, cudaStream_t st) {
 
 void reset_profile(Ctx* c) {
   c->launches = 0;
-  for (int s = 0; s < PM_NUM_STAGES; ++s) c->ev_used[s] = false;
+  c->ev_slot = 0;
+  for (int e = 0; e < 2; ++e)
+    for (int s = 0; s < PM_NUM_STAGES; ++s) c->ev_used[e][s] = false;
 }
 
 }  // namespace
@@ -322,6 +324,7 @@ int pm_force(pm_ctx* ctx, const float* pos, int64_t N, float* force, void* strea
   PM_TRY(bin_for_path(c, pos, N, st));
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
+    c->ev_slot = e;
     PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
     PM_TRY(gather_force(c, ev.sh[e], gather_values(3, nullptr, force, ev.weight, e == 0 ? 0.0f : 1.0f), st));
   }
@@ -344,6 +347,7 @@ int pm_force_vjp(pm_ctx* ctx, const float* pos, int64_t N, const float* force_co
   PM_TRY(bin_for_path(c, pos, N, st));  // returns at once when the pinned records are those of (pos, N)
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
+    c->ev_slot = e;
     if (!reuse) PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
     PM_TRY(vjp_from_meshes(c, N, ev.sh[e], ev.second_grid, force_cot, ev.weight, e == 0 ? 0.0f : 1.0f, pos_cot, st));
   }
@@ -370,6 +374,7 @@ int pm_dkd_step(pm_ctx* ctx, float* pos, float* vel, int64_t N, double tau1, dou
   PM_TRY(bin_for_path(c, pos, N, st));
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
+    c->ev_slot = e;
     PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
     // (2.14b) V <- alpha V + beta A in the gather epilogue; after the last evaluation (2.14c) X <- X + tau2 V
     GatherArgs ga = gather_values(3, nullptr, vel, (float)beta * ev.weight, e == 0 ? (float)alpha : 1.0f);
@@ -409,6 +414,7 @@ int pm_dkd_step_adjoint(pm_ctx* ctx, float* pos, float* vel, float* pos_adj, flo
   PM_TRY(bin_for_path(c, pos, N, st));
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
+    c->ev_slot = e;
     PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
     // primal kick V^{n-1} = (V^n - beta A) / alpha, with beta* = V*^{n-1/2} . A and (after the last evaluation)
     // alpha* = V*^{n-1/2} . V^{n-1} reduced in the same pass

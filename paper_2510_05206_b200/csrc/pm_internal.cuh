@@ -5,8 +5,11 @@
 //   * sorted particle records: one uint4 per particle {ux, uy, uz, orig_index}; u* are tile-local cell
 //     coordinates in unsigned fixed point, value = (u_local + REC_BIAS) * 2^REC_FRAC, computed once by the
 //     binning pass with an error-free product (the plain fp32 product x*(m/L) would cost 1e-5 of force
-//     accuracy).  (A structure-of-arrays layout was measured: the scatter read 0.4 GB less, but the permute
-//     pass took 1.29 ms instead of 0.69 ms -- four 128-byte write streams instead of one 512-byte one.)
+//     accuracy).  Two other layouts were measured and rejected: four separate arrays (round 1: the scatter read
+//     0.4 GB less, the permute pass took 1.29 ms instead of 0.69 ms) and word-transposed blocks of 32 records
+//     (round 2: ux[32] uy[32] uz[32] index[32] per 512 bytes; the assign read 12 B/particle and went 0.72 ->
+//     0.67 ms, but the binning pass, with four 4-byte stores per record, went 0.82 -> 1.21 ms at unchanged DRAM
+//     bytes -- its stall is the round trip of the slot-claim atomics, which the extra stores lengthen).
 //   * tiles of TX x TY x TZ cells in z-fastest order; tile_off[ntiles+1]; work items (tile, begin, end)
 //     of at most ITEM_MAX particles.
 #pragma once
@@ -58,12 +61,11 @@ __host__ __device__ __forceinline__ uint32_t tile_id(int tx, int ty, int tz, int
 
 enum { MAX_W = 16 };
 
-// Periodic wrap into [0, L) in fp32, operation by operation as DESIGN.md reading R18 specifies.
-__device__ __forceinline__ float wrap_box_fp32(float x, float L) {
-  float y = __fsub_rn(x, __fmul_rn(L, floorf(__fdiv_rn(x, L))));
+// Periodic wrap of a drifted coordinate into [0, L) in fp32, operation by operation as DESIGN.md reading R18 specifies
+// (one conditional add, then one conditional subtract; a particle moves less than one box length per drift).
+__device__ __forceinline__ float wrap_box_fp32(float y, float L) {
   if (y < 0.0f) y = __fadd_rn(y, L);
   if (y >= L) y = __fsub_rn(y, L);
-  if (y >= L || y < 0.0f) y = 0.0f;
   return y;
 }
 __device__ __forceinline__ float drift_fp32(float x, float v, float tau, float L) {
@@ -179,8 +181,9 @@ struct Ctx {
 
   // profiling
   bool profiling;
-  cudaEvent_t ev[2 * PM_NUM_STAGES];
-  bool ev_used[PM_NUM_STAGES];
+  cudaEvent_t ev[2][2 * PM_NUM_STAGES];  // [evaluation: interlace = 2 runs the stages twice][begin, end per stage]
+  bool ev_used[2][PM_NUM_STAGES];
+  int ev_slot;                           // evaluation the stages being recorded belong to
   bool ev_ok;
   int64_t launches;
   cudaStream_t prof_stream;
@@ -312,11 +315,8 @@ int spectral_potential_hat(Ctx* c, bool two, float2* out, double coeff_eff, cuda
 int spectral_potential(Ctx* c, const float* d1, const float* d2, float* phi, double coeff_eff, bool stages,
                        cudaStream_t st);
 int launch_xfft_potential(Ctx* c, const float2* d1, const float2* d2, float2* phi, double coeff_eff, cudaStream_t st);
-int launch_xfft_potential_tr(Ctx* c, const float2* psi, float2* q1, float2* q2, double coeff_eff, cudaStream_t st);
-int launch_kspace_scalar(Ctx* c, const float2* d1, const float2* d2, float2* q1, float2* q2, double coeff_eff, bool fwd,
-                         cudaStream_t st);
+int launch_kspace_scalar(Ctx* c, const float2* d1, const float2* d2, float2* q1, double coeff_eff, cudaStream_t st);
 int launch_fd_gradient(Ctx* c, const float* phi, float* const g[3], cudaStream_t st);
-int launch_fd_divergence(Ctx* c, const float* const gb[3], float* psi, cudaStream_t st);
 // forward-mode scatter (pm_jvp.cu)
 int launch_scatter_jvp(Ctx* c, int order, const ShiftSplit& sh, const float* w, const float* w_tan,
                        const float* pos_tan, float* mesh_tan, cudaStream_t st);

@@ -127,41 +127,32 @@ __global__ void __launch_bounds__(KS_BLOCK) k_kspace_tr(KTabs t, const float2* _
   }
 }
 
-// Scalar variants (no gradient symbol; PM_FLAG_GRAD_REAL / PM_FLAG_KERNEL_GRAD):
-//   fwd : q1 = green * (d2 ? 1/2 [d1 + e^{-ik.s} d2] : d1)                      (the potential's spectrum)
-//   !fwd: q1 = green * d1 (x 1/2 when q2), q2 = conj(e^{-ik.s}) q1                (its transpose; green is real, even)
+// Potential variant (no gradient symbol; PM_FLAG_GRAD_REAL / PM_FLAG_KERNEL_GRAD):
+//   q = green * (d2 ? 1/2 [d1 + e^{-ik.s} d2] : d1)
 __global__ void __launch_bounds__(KS_BLOCK) k_kspace_scalar(KTabs t, const float2* __restrict__ d1,
                                                             const float2* __restrict__ d2, float2* __restrict__ q1,
-                                                            float2* __restrict__ q2, double coeff_eff, int fwd) {
+                                                            double coeff_eff) {
   const int row0 = blockIdx.x * KS_ROWS;
   const int ix = row0 / t.m, iy0 = row0 - ix * t.m;
-  const bool phase = fwd ? d2 != nullptr : q2 != nullptr;
   RowFac rf[KS_ROWS];
 #pragma unroll
-  for (int r = 0; r < KS_ROWS; ++r) rf[r] = row_factors(t, ix, iy0 + r, phase, fwd ? 1.f : -1.f);
+  for (int r = 0; r < KS_ROWS; ++r) rf[r] = row_factors(t, ix, iy0 + r, d2 != nullptr, 1.f);
   const size_t base = (size_t)row0 * t.hz;
   for (int iz = threadIdx.x; iz < t.hz; iz += KS_BLOCK) {
     const double lz = t.lap[iz], wz = t.win[iz];
     float2 pz = make_float2(1.f, 0.f);
-    if (phase) pz = make_float2((float)t.pc[iz], (fwd ? 1.f : -1.f) * (float)t.ps[iz]);
+    if (d2) pz = make_float2((float)t.pc[iz], (float)t.ps[iz]);
 #pragma unroll
     for (int r = 0; r < KS_ROWS; ++r) {
       const size_t o = base + (size_t)r * t.hz + iz;
       const double den = (rf[r].lxy + lz) * (rf[r].wxy * wz);
       const float green = (float)((den != 0.0) ? coeff_eff / den : 0.0);
       float2 v = __ldcs(d1 + o);
-      if (fwd) {
-        if (d2) {
-          const float2 q = cmul(cmul(rf[r].pxy, pz), __ldcs(d2 + o));
-          v = make_float2(0.5f * (v.x + q.x), 0.5f * (v.y + q.y));
-        }
-        q1[o] = make_float2(green * v.x, green * v.y);
-      } else {
-        const float h = q2 ? 0.5f : 1.0f;
-        const float2 q = make_float2(h * green * v.x, h * green * v.y);
-        q1[o] = q;
-        if (q2) q2[o] = cmul(cmul(rf[r].pxy, pz), q);
+      if (d2) {
+        const float2 q = cmul(cmul(rf[r].pxy, pz), __ldcs(d2 + o));
+        v = make_float2(0.5f * (v.x + q.x), 0.5f * (v.y + q.y));
       }
+      q1[o] = make_float2(green * v.x, green * v.y);
     }
   }
 }
@@ -194,9 +185,8 @@ int launch_kspace_transpose(Ctx* c, const float2* const gh[3], float2* q1, float
   return PM_OK;
 }
 
-int launch_kspace_scalar(Ctx* c, const float2* d1, const float2* d2, float2* q1, float2* q2, double coeff_eff,
-                         bool fwd, cudaStream_t st) {
-  k_kspace_scalar<<<c->mg * c->mg / KS_ROWS, KS_BLOCK, 0, st>>>(tabs_of(c), d1, d2, q1, q2, coeff_eff, fwd ? 1 : 0);
+int launch_kspace_scalar(Ctx* c, const float2* d1, const float2* d2, float2* q1, double coeff_eff, cudaStream_t st) {
+  k_kspace_scalar<<<c->mg * c->mg / KS_ROWS, KS_BLOCK, 0, st>>>(tabs_of(c), d1, d2, q1, coeff_eff);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

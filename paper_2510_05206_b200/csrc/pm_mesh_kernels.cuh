@@ -27,6 +27,8 @@ struct PMTraits {
   static constexpr int HHI = (ORDER == 2 ? 1 : 2);
   // largest value of the 3-D kernel: W(0)^3 = 1 (CIC), (3/4)^3 (TSC), (2/3)^3 (PCS)
   static constexpr float WMAX3 = ORDER == 2 ? 1.0f : (ORDER == 3 ? 0.421875f : 0.2962963f);
+  // largest value of |dW/du| W W: 1 (CIC), 1 * (3/4)^2 (TSC), (2/3)^3 (PCS: max|W'| = 2/3 at |x| = 2/3)
+  static constexpr float DWMAX3 = ORDER == 2 ? 1.0f : (ORDER == 3 ? 0.5625f : 0.2962963f);
   struct Params {
     uint32_t frac[3];
   };
@@ -76,6 +78,7 @@ struct ESTraits {
   static constexpr int HLO = ODD ? (W - 1) / 2 : W / 2 - 1;
   static constexpr int HHI = ODD ? (W + 1) / 2 : W / 2;
   static constexpr float WMAX3 = 1.0f;  // phi(0) = 1
+  static constexpr float DWMAX3 = 1.0f; // (forward-mode scatter is not instantiated for the ES kernel)
   struct Params {
     uint32_t frac[3];  // unused (no shift), kept for a uniform interface
     float beta;
@@ -221,7 +224,16 @@ __device__ __forceinline__ uint32_t atom_inc_raw(uint32_t* p) {
   asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(r) : "l"(p) : "memory");
   return r;
 }
-__device__ __forceinline__ uint32_t sched_next(uint32_t* sched) { return gridDim.x + atom_inc_raw(&sched[0]); }
+// ptxas ALSO aggregates the raw add when it can prove the address warp-uniform (VOTEU / POPC / ATOMG.ADD / SHFL.IDX:
+// ncu round 2 showed 9 % of the warp-private scatter's stall samples on that SHFL, once per work item).  The wrapping
+// increment atom.inc has no popcount form, so it stays a plain per-thread ATOMG whose result is first touched where
+// the caller reads it (the bound 2^31 - 1 is never reached: the counter counts work items; with the bound 2^32 - 1 ptxas turns inc back into add).
+__device__ __forceinline__ uint32_t atom_inc_noagg(uint32_t* p) {
+  uint32_t r;
+  asm volatile("atom.global.inc.u32 %0, [%1], 2147483647;" : "=r"(r) : "l"(p) : "memory");
+  return r;
+}
+__device__ __forceinline__ uint32_t sched_next(uint32_t* sched) { return gridDim.x + atom_inc_noagg(&sched[0]); }
 __device__ __forceinline__ void sched_done(uint32_t* sched) {
   if (atomicAdd(&sched[1], 1u) == gridDim.x - 1u) {
     sched[0] = 0u;
@@ -234,6 +246,7 @@ template <bool IDX>  // IDX: the caller reads the original index (.w)
 __device__ __forceinline__ void load_rec(uint4& r, const BinView& bv, uint32_t i) {
   r = __ldcs(bv.rec + i);
 }
+__device__ __forceinline__ uint32_t rec_index(const BinView& bv, uint32_t i) { return bv.rec[i].w; }
 
 // ---- K2 / K5: tile scatter ---------------------------------------------------------------------------
 // Persistent CTAs draw work items from the dynamic schedule, two items ahead: while item i is deposited, the
@@ -324,7 +337,7 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
     // item i+2: the atomic is issued now and its result is only touched right before the barrier below (stored
     // at once, thread 0 would wait ~microseconds for the contended counter with the whole CTA behind it)
     uint32_t fetched = 0;
-    if (tid == 0) fetched = sched_next(bv.sched);
+    if (tid == 0) fetched = atom_inc_noagg(&bv.sched[0]);  // raw: gridDim.x is added where it is stored
     const uint32_t n = wi.end - wi.begin;
     const uint32_t ibegin = wi.begin, iend = wi.end;
     const TileOrigin o = tile_origin(wi);
@@ -346,8 +359,8 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
         }
         const float ws = w * src.tan_scale;
         pv[1] = ws * t0, pv[2] = ws * t1, pv[3] = ws * t2;
-        // |W| <= 1 and |dW/du| <= 1 for the kernels of Table 1
-        wabs[0] += fabsf(pv[0]) + fabsf(pv[1]) + fabsf(pv[2]) + fabsf(pv[3]);
+        // largest deposit of a particle: |w~| W_max^3 + |w t|_1 max|dW/du| W_max^2 (Table 1: CIC 1, TSC 9/16, PCS 8/27)
+        wabs[0] += fabsf(pv[0]) * T::WMAX3 + (fabsf(pv[1]) + fabsf(pv[2]) + fabsf(pv[3])) * T::DWMAX3;
       } else {
 #pragma unroll
         for (int a = 0; a < NCOMP; ++a) {
@@ -367,7 +380,7 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
     if (WEIGHTED && n > (uint32_t)CHUNK) {  // dense tile: the bound needs the weights of the later batches too
       for (uint32_t i = ibegin + CHUNK + tid; i < iend; i += BLOCK) {
         float pv[NPAY];
-        payload(bv.rec[i].w, pv);
+        payload(rec_index(bv, i), pv);
       }
     }
 
@@ -480,7 +493,7 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
       load_batch(b0, iend);  // dense tile: further batches of the same item
       load_weights(b0);
     }
-    if (tid == 0) s_next[par] = fetched;
+    if (tid == 0) s_next[par] = fetched + gridDim.x;
     __syncthreads();
     const uint32_t nn = s_next[par];
     par ^= 1;
@@ -547,9 +560,6 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
 constexpr int WS_WARPS = 4;  // warps per CTA
 constexpr int WD = 10;       // records in flight per lane (128 registers per thread at 4 CTAs of 128 threads)
 
-__device__ __forceinline__ uint32_t wsched_next(uint32_t* sched, uint32_t nwarps) {
-  return nwarps + atom_inc_raw(&sched[0]);
-}
 __device__ __forceinline__ void wsched_done(uint32_t* sched, uint32_t nwarps) {
   if (atomicAdd(&sched[1], 1u) == nwarps - 1u) {
     sched[0] = 0u;
@@ -559,12 +569,11 @@ __device__ __forceinline__ void wsched_done(uint32_t* sched, uint32_t nwarps) {
 
 template <class T, bool FASTCIC>
 __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, typename T::Params tp, int3 roll,
-                                                                   float* __restrict__ mesh, int zeroed) {
+                                                                   float* __restrict__ mesh, int zeroed, uint32_t wb) {
   using G = Geo<T>;
   constexpr int P = T::P;
   constexpr int NG = G::NGROUP;
   extern __shared__ __align__(16) int s_acc_all[];
-  __shared__ volatile uint32_t s_mail[WS_WARPS];
   const unsigned lane = threadIdx.x & 31u;
   int* s_acc = s_acc_all + (threadIdx.x >> 5) * G::COMP;
   const uint32_t nitems = *bv.nitems;
@@ -574,9 +583,24 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
   for (int j = (int)lane; j < G::COMP / 4; j += 32) reinterpret_cast<int4*>(s_acc)[j] = make_int4(0, 0, 0, 0);
   __syncwarp();
 
-  uint32_t it = blockIdx.x * WS_WARPS + (threadIdx.x >> 5), nxt = 0;
-  if (lane == 0) nxt = wsched_next(bv.sched, nwarps);
-  nxt = __shfl_sync(0xffffffffu, nxt, 0);
+  // Dynamic schedule in BATCHES of wb consecutive work items: warp g starts with batch g, further batches come
+  // from the global counter.  The counter's round trip is long when every warp of the grid hammers it (one
+  // same-address atomic per item: on the oversampled meshes, 256 particles per item, ncu round 2 showed 56 % of the
+  // stall samples waiting for it, whatever instruction touched the result first), so (i) a batch is requested when
+  // the previous one is STARTED and its id is first touched wb items later, (ii) wb = 8 items per request when the
+  // items are light; wb = 1 for the heavy items of the headline, where balance matters more (host: run_scatter_warp).
+  uint32_t q = (blockIdx.x * WS_WARPS + (threadIdx.x >> 5)) * wb, qend = q + wb;
+  uint32_t claim = 0;  // lane 0: raw counter value = index of the next batch minus nwarps
+  if (lane == 0) claim = atom_inc_noagg(&bv.sched[0]);
+  auto next_id = [&]() -> uint32_t {  // warp-uniform
+    if (q == qend) {
+      q = (__shfl_sync(0xffffffffu, claim, 0) + nwarps) * wb;
+      qend = q + wb;
+      if (lane == 0) claim = atom_inc_noagg(&bv.sched[0]);
+    }
+    return q++;
+  };
+  uint32_t it = next_id(), nxt = next_id();
   WorkItem wi, nwi;
   wi.begin = wi.end = wi.txyz = nwi.begin = nwi.end = nwi.txyz = 0;
   uint4 r[WD];
@@ -594,8 +618,7 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
   if (nxt < nitems) nwi = bv.items[nxt];
 
   while (it < nitems) {
-    uint32_t nn = 0;
-    if (lane == 0) nn = wsched_next(bv.sched, nwarps);  // item i+2; consumed after the deposit
+    const uint32_t nn = next_id();  // item i+2
     const uint32_t n = wi.end - wi.begin;
     const uint32_t iend = wi.end;
     const TileOrigin o = tile_origin(wi);
@@ -644,18 +667,17 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
             atomicAdd(p0 + (G::SY + 1) * TZ, __float2uint_rn(w11 * ozs));
             const unsigned u00 = __float2uint_rn(w00 * tzs), u01 = __float2uint_rn(w01 * tzs);
             const unsigned u10 = __float2uint_rn(w10 * tzs), u11 = __float2uint_rn(w11 * tzs);
-            if (sz < TZ - 1) {
-              atomicAdd(p0 + 1, u00);
-              atomicAdd(p0 + TZ + 1, u01);
-              atomicAdd(p0 + G::SY * TZ + 1, u10);
-              atomicAdd(p0 + (G::SY + 1) * TZ + 1, u11);
-            } else {
-              unsigned* ph = reinterpret_cast<unsigned*>(s_acc) + (G::MAIN + row0 * G::HZ);
-              atomicAdd(ph, u00);
-              atomicAdd(ph + G::HZ, u01);
-              atomicAdd(ph + G::SY * G::HZ, u10);
-              atomicAdd(ph + (G::SY + 1) * G::HZ, u11);
-            }
+            // second z node: next word of the MAIN plane, or (sz = TZ - 1) the first column of the HALO plane, whose
+            // rows have another pitch.  Selected, not branched: with 32 lanes at 32 different z one lane of almost
+            // every warp is at sz = TZ - 1, and the branch made 64 % of the warps run both sides (ncu round 2: 10.6
+            // instead of 8 ATOMS per warp and particle, and the shared-memory pipe is the busiest unit, 66 %).
+            const bool inm = sz < TZ - 1;
+            unsigned* p1 = inm ? p0 + 1 : reinterpret_cast<unsigned*>(s_acc) + (G::MAIN + row0 * G::HZ);
+            const int py = inm ? TZ : G::HZ, px = inm ? G::SY * TZ : G::SY * G::HZ;
+            atomicAdd(p1, u00);
+            atomicAdd(p1 + py, u01);
+            atomicAdd(p1 + px, u10);
+            atomicAdd(p1 + px + py, u11);
             continue;
           }
           int sx, sy, sz;
@@ -683,12 +705,7 @@ __global__ void __launch_bounds__(WS_WARPS * 32, 4) k_scatter_warp(BinView bv, t
       }
       if (last) break;
     }
-    // The counter's value travels through a shared-memory mailbox, not a shuffle: ptxas hoisted the shuffle to
-    // right behind the atomic and the warp sat out the contended counter's round trip once per item (ncu: 18 %
-    // of the stall samples on that SHFL).  The store cannot move above the shared-memory atomics of the deposit.
-    if (lane == 0) s_mail[threadIdx.x >> 5] = nn;
-    __syncwarp();  // the lanes' deposits (and the mailbox) are visible below
-    nn = s_mail[threadIdx.x >> 5];
+    __syncwarp();  // the lanes' deposits are visible below
     WorkItem nnwi = nwi;
     if (nn < nitems) nnwi = bv.items[nn];
 
@@ -891,7 +908,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   while (it < nitems) {
     uint32_t fetched = 0;  // item i+2: issued now, stored right before the barrier at the end of the item
     if (tid == 0) {
-      fetched = sched_next(bv.sched);
+      fetched = atom_inc_noagg(&bv.sched[0]);  // raw: gridDim.x is added where it is stored
       if (STAGES == 2 && nxt < nitems) issue(nwi, stage ^ 1);
     }
     const TileOrigin o = tile_origin(wi);
@@ -1042,7 +1059,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
       }
       if (last) break;
     }
-    if (tid == 0) s_next[par] = fetched;
+    if (tid == 0) s_next[par] = fetched + gridDim.x;
     __syncthreads();  // every thread is done with this stage: it may be refilled
     const uint32_t nn = s_next[par];
     par ^= 1;
@@ -1132,8 +1149,11 @@ int run_scatter_warp(Ctx* c, const typename T::Params& tp, const int roll[3], fl
   const int64_t bound = ((int64_t)c->ntiles + c->bin_n / ITEM_MAX + 1 + WS_WARPS - 1) / WS_WARPS;
   const int64_t cap = (int64_t)c->num_sms * occ;
   const int m = c->mg;
+  // work items per schedule request: light items (oversampled meshes) in batches of up to 8, heavy ones singly
+  const int64_t per_item = c->bin_n / (c->ntiles > 0 ? c->ntiles : 1);
+  const uint32_t wb = per_item >= 1024 ? 1u : (per_item >= 512 ? 2u : (per_item >= 256 ? 4u : 8u));
   kern<<<(int)(bound < cap ? bound : cap), WS_WARPS * 32, smem, st>>>(
-      bin_view(c), tp, make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m)), mesh, zeroed);
+      bin_view(c), tp, make_int3(norm_roll(roll[0], m), norm_roll(roll[1], m), norm_roll(roll[2], m)), mesh, zeroed, wb);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

@@ -2,13 +2,15 @@
 // ("Real" column: 1/2 [-1 0 1], 1/12 [1 -8 0 8 -1], 1/60 [-1 9 -45 0 45 -9 1]; the "Fourier"
 // column is the DFT of these stencils, so IFFT(-i D(theta)/Delta phi_hat) == -stencil(IFFT(phi_hat))).
 //
-//   k_fd_gradient  : phi -> g_a = -(1/Delta) sum_s c_s (phi[j + s e_a] - phi[j - s e_a]),  a = x, y, z   (forward)
-//   k_fd_divergence: gbar_a -> psi = sum_a (1/Delta) sum_s c_s (gbar_a[j + s e_a] - gbar_a[j - s e_a])    (transpose:
-//                    the stencil is antisymmetric, D^T = -D, so (-D_a K)^T gbar = K sum_a D_a gbar_a)
+//   k_fd_gradient  : phi -> g_a = -(1/Delta) sum_s c_s (phi[j + s e_a] - phi[j - s e_a]),  a = x, y, z
 //
-// One inverse FFT instead of three for the force (and one forward FFT instead of three for the VJP): the
-// Fourier-space kernel writes 4G instead of 12G bytes, two C2R (R2C) transforms disappear, and this pass moves
-// 4G + 12G.  HBM-bound: a CTA owns a (YB x ZB) patch of one x plane; the z and y neighbours come from L1, the
+// One inverse FFT instead of three for the force: the Fourier-space kernel writes 4G instead of 12G bytes, two C2R
+// transforms disappear, and this pass moves 4G + 12G.  The TRANSPOSED operator (VJP) stays in Fourier space: the
+// real-space form, psi = sum_a D_a gbar_a followed by ONE forward transform, was built and measured -- parity
+// 4e-6 at 64^3 but 1.9e-5 at 512^3: the cotangent meshes are rough (scattered lambda), storing their divergence in
+// fp32 injects WHITE rounding noise, while the wanted signal i D(k) gbar_hat vanishes like k at low k, exactly
+// where the Green's function 1/k^2 then puts its weight; in Fourier space the rounding error of a mode is scaled
+// by D(k) with the mode.  The forward direction differentiates the SMOOTH potential and has no such problem.  HBM-bound: a CTA owns a (YB x ZB) patch of one x plane; the z and y neighbours come from L1, the
 // x neighbours from L2 (2R + 1 planes of m^2 floats are live at a time: 5 MB at m = 512, FD4).
 #include "pm_internal.cuh"
 
@@ -85,30 +87,6 @@ __global__ void __launch_bounds__(SB) k_fd_gradient(const float* __restrict__ ph
   __stcs(reinterpret_cast<float4*>(gz + o), make_float4(k * az.x, k * az.y, k * az.z, k * az.w));
 }
 
-template <int R>
-__global__ void __launch_bounds__(SB) k_fd_divergence(const float* __restrict__ bx, const float* __restrict__ by,
-                                                      const float* __restrict__ bz, float* __restrict__ psi, int m,
-                                                      float inv_delta) {
-  const int z = (blockIdx.x * ZV + (threadIdx.x % ZV)) * 4;
-  const int y = blockIdx.y * YB + threadIdx.x / ZV;
-  const int x = blockIdx.z;
-  if (z >= m || y >= m) return;
-  const size_t mm = (size_t)m * m;
-  const float* row = bz + (size_t)x * mm + (size_t)y * m;
-  float4 acc = zdiff<R>(ld4(row + wrapi(z - 4, m)), ld4(row + z), ld4(row + wrapi(z + 4, m)));
-#pragma unroll
-  for (int s = 1; s <= R; ++s) {
-    const float c = fd_coef(R, s);
-    acc = fma4(c, sub4(ld4(bx + (size_t)wrapi(x + s, m) * mm + (size_t)y * m + z),
-                       ld4(bx + (size_t)wrapi(x - s, m) * mm + (size_t)y * m + z)), acc);
-    acc = fma4(c, sub4(ld4(by + (size_t)x * mm + (size_t)wrapi(y + s, m) * m + z),
-                       ld4(by + (size_t)x * mm + (size_t)wrapi(y - s, m) * m + z)), acc);
-  }
-  const float k = inv_delta;
-  __stcs(reinterpret_cast<float4*>(psi + (size_t)x * mm + (size_t)y * m + z),
-         make_float4(k * acc.x, k * acc.y, k * acc.z, k * acc.w));
-}
-
 dim3 stencil_grid(int m) { return dim3((m / 4 + ZV - 1) / ZV, (m + YB - 1) / YB, m); }
 
 }  // namespace
@@ -121,21 +99,6 @@ int launch_fd_gradient(Ctx* c, const float* phi, float* const g[3], cudaStream_t
     case 2: k_fd_gradient<1><<<stencil_grid(m), SB, 0, st>>>(phi, g[0], g[1], g[2], m, k); break;
     case 4: k_fd_gradient<2><<<stencil_grid(m), SB, 0, st>>>(phi, g[0], g[1], g[2], m, k); break;
     case 6: k_fd_gradient<3><<<stencil_grid(m), SB, 0, st>>>(phi, g[0], g[1], g[2], m, k); break;
-    default: return fail(c, PM_ESTATE, "real-space gradient needs grad_order 2, 4 or 6");
-  }
-  count_launch(c);
-  PM_CUDA(c, cudaGetLastError());
-  return PM_OK;
-}
-
-// psi = sum_a D_a gbar_a (the transpose of g = -D K delta is delta_bar = K psi)
-int launch_fd_divergence(Ctx* c, const float* const gb[3], float* psi, cudaStream_t st) {
-  const int m = c->mg;
-  const float k = (float)((double)m / c->p.box);
-  switch (c->p.grad_order) {
-    case 2: k_fd_divergence<1><<<stencil_grid(m), SB, 0, st>>>(gb[0], gb[1], gb[2], psi, m, k); break;
-    case 4: k_fd_divergence<2><<<stencil_grid(m), SB, 0, st>>>(gb[0], gb[1], gb[2], psi, m, k); break;
-    case 6: k_fd_divergence<3><<<stencil_grid(m), SB, 0, st>>>(gb[0], gb[1], gb[2], psi, m, k); break;
     default: return fail(c, PM_ESTATE, "real-space gradient needs grad_order 2, 4 or 6");
   }
   count_launch(c);

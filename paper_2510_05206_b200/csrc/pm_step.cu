@@ -18,21 +18,42 @@ namespace {
 
 constexpr int STB = 256;
 
-// n3 = 3N scalars.  xs == NULL: drift only.
+// n3 = 3N scalars, VEC of them per thread and iteration (VEC = 4: 16-byte accesses).  xs == NULL: drift only.
+template <int VEC>
 __global__ void __launch_bounds__(STB) k_step_update(float* __restrict__ x, const float* __restrict__ v,
                                                      const float* __restrict__ xs, float* __restrict__ vs, int64_t n3,
                                                      float tau_x, float a, float b, float box,
                                                      double* __restrict__ dot) {
   __shared__ double s_part[STB / 32];
   double acc = 0.0;
-  const int64_t stride = (int64_t)gridDim.x * STB;
-  for (int64_t i = (int64_t)blockIdx.x * STB + threadIdx.x; i < n3; i += stride) {
-    const float vi = __ldcs(v + i);
-    x[i] = drift_fp32(__ldcs(x + i), vi, tau_x, box);
-    if (xs) {
-      const float xsi = __ldcs(xs + i);
-      vs[i] = fmaf(b, xsi, a * __ldcs(vs + i));
-      acc += (double)xsi * (double)vi;
+  const int64_t stride = (int64_t)gridDim.x * STB * VEC;
+  for (int64_t i = ((int64_t)blockIdx.x * STB + threadIdx.x) * VEC; i < n3; i += stride) {
+    float xv[VEC], vv[VEC], xsv[VEC], vsv[VEC];
+    if (VEC == 4) {
+      *reinterpret_cast<float4*>(xv) = __ldcs(reinterpret_cast<const float4*>(x + i));
+      *reinterpret_cast<float4*>(vv) = __ldcs(reinterpret_cast<const float4*>(v + i));
+      if (xs) {
+        *reinterpret_cast<float4*>(xsv) = __ldcs(reinterpret_cast<const float4*>(xs + i));
+        *reinterpret_cast<float4*>(vsv) = __ldcs(reinterpret_cast<const float4*>(vs + i));
+      }
+    } else {
+      xv[0] = x[i], vv[0] = v[i];
+      if (xs) xsv[0] = xs[i], vsv[0] = vs[i];
+    }
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) {
+      xv[k] = drift_fp32(xv[k], vv[k], tau_x, box);
+      if (xs) {
+        vsv[k] = fmaf(b, xsv[k], a * vsv[k]);
+        acc += (double)xsv[k] * (double)vv[k];
+      }
+    }
+    if (VEC == 4) {
+      *reinterpret_cast<float4*>(x + i) = *reinterpret_cast<float4*>(xv);
+      if (xs) *reinterpret_cast<float4*>(vs + i) = *reinterpret_cast<float4*>(vsv);
+    } else {
+      x[i] = xv[0];
+      if (xs) vs[i] = vsv[0];
     }
   }
   if (xs && dot) {
@@ -54,10 +75,17 @@ int launch_step_update(Ctx* c, float* x, const float* v, const float* xs, float*
                        float b, double* dot, cudaStream_t st) {
   const int64_t n3 = 3 * n;
   if (n3 == 0) return PM_OK;
-  int64_t grid = (n3 + STB - 1) / STB;
+  const uintptr_t al = reinterpret_cast<uintptr_t>(x) | reinterpret_cast<uintptr_t>(v) |
+                       reinterpret_cast<uintptr_t>(xs) | reinterpret_cast<uintptr_t>(vs);
+  const bool vec = (n3 % 4 == 0) && (al & 15u) == 0;
+  const int64_t work = vec ? n3 / 4 : n3;
+  int64_t grid = (work + STB - 1) / STB;
   const int64_t cap = (int64_t)c->num_sms * 8;
   if (grid > cap) grid = cap;
-  k_step_update<<<(unsigned)grid, STB, 0, st>>>(x, v, xs, vs, n3, tau_x, a, b, (float)c->p.box, dot);
+  if (vec)
+    k_step_update<4><<<(unsigned)grid, STB, 0, st>>>(x, v, xs, vs, n3, tau_x, a, b, (float)c->p.box, dot);
+  else
+    k_step_update<1><<<(unsigned)grid, STB, 0, st>>>(x, v, xs, vs, n3, tau_x, a, b, (float)c->p.box, dot);
   count_launch(c);
   PM_CUDA(c, cudaGetLastError());
   return PM_OK;

@@ -239,7 +239,6 @@ struct XTabs {
 //   MODE 2 (potential): in0 (, in1) -> out0 = x-inverse of green(n) dhat(n): no gradient symbol -- the gradient is
 //                       applied in real space (PM_FLAG_GRAD_REAL, pm_stencil.cu) or by the interpolation kernel
 //                       (PM_FLAG_KERNEL_GRAD)
-//   MODE 3 (its transpose): in0 -> out0 (, out1) = x-inverse of green(n) in0(n) (x 1/2, x conj phase for out1)
 // Every input is the (y,z)-transformed, x-untransformed spectrum [x][y][hz]; every output likewise.
 template <int N, int MODE>
 __global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? (XEPT >= 16 ? 3 : 2) : 1) k_xfft_kspace(XTabs t, const float2* __restrict__ in0,
@@ -341,23 +340,6 @@ __global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? (XEPT >= 16 ? 3 : 2) 
       s_a[sidx(p, cc)] = make_float2(g * v.x, g * v.y);
     });
     xfft_line<N, true>(s_w, t.tw, tid, [&](int p, int cc) { return s_a[sidx(p, cc)]; }, gst(out0));
-  } else if (MODE == 3) {
-    const bool two = out1 != nullptr;
-    xfft_line<N, false>(s_w, t.tw, tid, gld(in0), [&](int p, int cc, float2 v) { s_a[sidx(p, cc)] = v; });
-#pragma unroll 1
-    for (int o = 0; o < (two ? 2 : 1); ++o) {
-      xfft_line<N, true>(
-          s_w, t.tw, tid,
-          [&](int p, int cc) {
-            const int kx = xfft_freq<N>(p);
-            const float g = green_of(kx) * (two ? 0.5f : 1.0f);
-            const float2 d = s_a[sidx(p, cc)];
-            float2 v = make_float2(g * d.x, g * d.y);
-            if (o == 1) v = cmulc(v, phase_of(kx));
-            return v;
-          },
-          gst(o == 0 ? out0 : out1));
-    }
   } else {
     const bool two = out1 != nullptr;
     // conj(S_a) = +i D_a green:  q = i [D_x FFT_x(g_x) + FFT_x(D_y g_y + D_z g_z)]; green is applied on the way
@@ -506,12 +488,9 @@ int launch_xfft_transpose(Ctx* c, const float2* const gh[3], float2* q1, float2*
   return xfft_launch<1>(c, gh[0], gh[1], gh[2], q1, q2, nullptr, coeff_eff, st);
 }
 
-// potential: d1 (, d2) -> phi spectrum;  its transpose: psi spectrum -> q1 (, q2)
+// potential: d1 (, d2) -> phi spectrum
 int launch_xfft_potential(Ctx* c, const float2* d1, const float2* d2, float2* phi, double coeff_eff, cudaStream_t st) {
   return xfft_launch<2>(c, d1, d2, nullptr, phi, nullptr, nullptr, coeff_eff, st);
-}
-int launch_xfft_potential_tr(Ctx* c, const float2* psi, float2* q1, float2* q2, double coeff_eff, cudaStream_t st) {
-  return xfft_launch<3>(c, psi, nullptr, nullptr, q1, q2, nullptr, coeff_eff, st);
 }
 
 // ---- the spectral operator on real meshes, fused or not ------------------------------------------------------
@@ -550,7 +529,7 @@ int spectral_forward(Ctx* c, const float* d1, const float* d2, float* const g[3]
 // dhat[0] (, dhat[1]) -> out = green * (combined) density spectrum (x-inverse-transformed on the fused path)
 int spectral_potential_hat(Ctx* c, bool two, float2* out, double coeff_eff, cudaStream_t st) {
   if (c->xfused) return launch_xfft_potential(c, c->dhat[0], two ? c->dhat[1] : nullptr, out, coeff_eff, st);
-  return launch_kspace_scalar(c, c->dhat[0], two ? c->dhat[1] : nullptr, out, nullptr, coeff_eff, true, st);
+  return launch_kspace_scalar(c, c->dhat[0], two ? c->dhat[1] : nullptr, out, coeff_eff, st);
 }
 
 // The potential mesh of the spread / assigned density: d1 (, d2) -> phi (real space).  Used by the NUFFT
@@ -571,23 +550,15 @@ int spectral_potential(Ctx* c, const float* d1, const float* d2, float* phi, dou
   return PM_OK;
 }
 
+// The transposed operator always works in Fourier space, also for a PM_FLAG_GRAD_REAL ctx (same linear operator;
+// see pm_stencil.cu for why its real-space form is not used).
 int spectral_transpose(Ctx* c, const float* const gb[3], float* q1, float* q2, double coeff_eff, cudaStream_t st) {
   const bool fused = c->xfused;
-  if (c->p.flags & PM_FLAG_GRAD_REAL) {  // psi = sum_a D_a gbar_a in real space, then ONE forward transform
-    PM_TRY(ensure_phi(c));
-    PM_TRY(launch_fd_divergence(c, gb, c->phi, st));
-    PM_TRY(fused ? fft2_r2c(c, c->phi, c->ghat[0], st) : fft_r2c(c, c->phi, c->ghat[0], st));
-    if (fused)
-      PM_TRY(launch_xfft_potential_tr(c, c->ghat[0], c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, st));
-    else
-      PM_TRY(launch_kspace_scalar(c, c->ghat[0], nullptr, c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, false, st));
-  } else {
-    for (int a = 0; a < 3; ++a) PM_TRY(fused ? fft2_r2c(c, gb[a], c->ghat[a], st) : fft_r2c(c, gb[a], c->ghat[a], st));
-    if (fused)
-      PM_TRY(launch_xfft_transpose(c, c->ghat, c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, st));
-    else
-      PM_TRY(launch_kspace_transpose(c, c->ghat, c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, st));
-  }
+  for (int a = 0; a < 3; ++a) PM_TRY(fused ? fft2_r2c(c, gb[a], c->ghat[a], st) : fft_r2c(c, gb[a], c->ghat[a], st));
+  if (fused)
+    PM_TRY(launch_xfft_transpose(c, c->ghat, c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, st));
+  else
+    PM_TRY(launch_kspace_transpose(c, c->ghat, c->dhat[0], q2 ? c->dhat[1] : nullptr, coeff_eff, st));
   PM_TRY(fused ? fft2_c2r(c, c->dhat[0], q1, st) : fft_c2r(c, c->dhat[0], q1, st));
   if (q2) PM_TRY(fused ? fft2_c2r(c, c->dhat[1], q2, st) : fft_c2r(c, c->dhat[1], q2, st));
   return PM_OK;

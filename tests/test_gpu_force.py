@@ -266,3 +266,27 @@ def test_pm_force_host_matches_device(pm):
     ms, launches = pm.pm_get_stage_ms(ctx)
     assert launches >= 8 and ms["assign"] > 0 and ms["interp"] > 0
     pm.pm_destroy(ctx)
+
+
+def test_run_to_run_spread(pm):
+    """Atomics make the summation order, hence the fp32 result, vary from run to run.
+    The fixed-point tile accumulators are order-independent, so only the global reductions on tile faces and cuFFT
+    contribute: the spread of 10 runs must stay below a tenth of the parity budget."""
+    pos, c = gen.make_config_positions("cfg1")
+    n = pos.shape[0]
+    ctx = pm.pm_create(params_of(pm, c, n))
+    d_pos = dev(pos)
+    lam = dev(gen.gaussian_cotangent(n, c["cot_seed"]))
+    runs, runs_v = [], []
+    for _ in range(10):
+        f, xb = torch.empty(n, 3, device="cuda"), torch.empty(n, 3, device="cuda")
+        pm.pm_force(ctx, d_pos, f)
+        pm.pm_force_vjp(ctx, d_pos, lam, xb)
+        runs.append(f)
+        runs_v.append(xb)
+    pm.pm_destroy(ctx)
+    for name, rs in (("force", runs), ("vjp", runs_v)):
+        ref = rs[0].double()
+        spread = max(float((r.double() - ref).norm() / ref.norm()) for r in rs[1:])
+        record_error(f"run_to_run_spread/cfg1/{name}", spread, 1e-6)
+        assert spread <= 1e-6, (name, spread)

@@ -115,7 +115,7 @@ def test_fp32_state_drift_arithmetic():
     """Reading R18: the fp32 drift wraps into [0, L) and keeps fp32 bits; a value that rounds to L becomes 0."""
     box = 1000.0
     X = np.array([[999.99994, 0.0, 500.0], [1e-6, 999.0, 3.0]], dtype=np.float32)
-    V = np.array([[1.0, -1.0, 0.0], [-1.0, 2.0, 1e4]], dtype=np.float32)
+    V = np.array([[1.0, -1.0, 0.0], [-1.0, 2.0, 1.9e3]], dtype=np.float32)
     Y = dk.drift(X, V, 0.5, box, np.float32)
     assert Y.dtype == np.float32 and (Y >= 0).all() and (Y < np.float32(box)).all()
     ref = np.mod(X.astype(np.float64) + 0.5 * V.astype(np.float64), box)

@@ -69,7 +69,8 @@ typedef struct pm_params {
 #define PM_FLAG_GRAD_REAL 4   /* a3-a4, method 0, grad_order 2/4/6: apply the gradient as the real-space stencil of
                                  Table 2 ("Real" column; its DFT IS the Fourier symbol) to the
                                  potential mesh: ONE inverse FFT instead of three.  Same operator, other rounding.
-                                 The transposed operator (VJP) keeps the Fourier-space form. */
+                                 Forward evaluations only (pm_force, pm_dkd_step, pm_poisson_force): the reverse-mode
+                                 calls always use the Fourier-space operator. */
 #define PM_FLAG_KERNEL_GRAD 8 /* method 1: force from the gradient of the ES kernel ("SPH-like"):
                                  the potential is interpolated with grad(phi_ES) instead of multiplying by i k.
                                  pm_force only (its VJP would need second derivatives of the kernel: PM_ESTATE). */

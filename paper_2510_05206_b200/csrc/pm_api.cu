@@ -67,7 +67,12 @@ int gather_any(Ctx* c, const ShiftSplit& sh, const GatherArgs& a, cudaStream_t s
 // a1-a4 on the grid shifted by `sh`: the binned particles -> force meshes g[0..2] (or, for the NUFFT
 // kernel-gradient option, the potential mesh phi).  coeff_eff carries every scalar: coeff, the density-contrast
 // factor m^3/N of Eq. 2.3 and cuFFT's missing 1/m^3.
-int forward_meshes(Ctx* c, int64_t N, const ShiftSplit& sh, bool second_grid, cudaStream_t st) {
+// for_vjp: the meshes feed grad-W gathers (the direct term of the VJP, Eq. C.12), which difference g between
+// neighbouring nodes.  The real-space stencil of PM_FLAG_GRAD_REAL leaves white rounding noise eps |phi| / Delta on g
+// (phi is dominated by low k and much larger than Delta |grad phi|): harmless for the force itself (1e-6), amplified
+// by that second difference (measured 1.85e-5 on the VJP at 512^3, 4e-6 at 64^3).  Reverse-mode calls therefore
+// always take the three-inverse-FFT meshes, whatever the flag says.
+int forward_meshes(Ctx* c, int64_t N, const ShiftSplit& sh, bool second_grid, bool for_vjp, cudaStream_t st) {
   c->g_valid = false;
   PM_TRY(assign_ctx_meshes(c, sh, second_grid, st));
   const double coeff_eff = c->p.coeff / (double)N;
@@ -75,7 +80,11 @@ int forward_meshes(Ctx* c, int64_t N, const ShiftSplit& sh, bool second_grid, cu
     PM_TRY(ensure_phi(c));
     return spectral_potential(c, c->rho[0], nullptr, c->phi, coeff_eff, true, st);
   }
-  return spectral_forward(c, c->rho[0], second_grid ? c->rho[1] : nullptr, c->g, coeff_eff, true, st);
+  const int32_t flags = c->p.flags;
+  if (for_vjp) c->p.flags &= ~PM_FLAG_GRAD_REAL;
+  const int rc = spectral_forward(c, c->rho[0], second_grid ? c->rho[1] : nullptr, c->g, coeff_eff, true, st);
+  c->p.flags = flags;
+  return rc;
 }
 
 // a5: per-particle values of the force meshes with the epilogue of `ga` (out = alpha * A + out_scale * out, ...)
@@ -325,11 +334,11 @@ int pm_force(pm_ctx* ctx, const float* pos, int64_t N, float* force, void* strea
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
     c->ev_slot = e;
-    PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
+    PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, false, st));
     PM_TRY(gather_force(c, ev.sh[e], gather_values(3, nullptr, force, ev.weight, e == 0 ? 0.0f : 1.0f), st));
   }
-  // the meshes stay valid for a pm_force_vjp on the same pinned records (a single evaluation only)
-  c->g_valid = ev.n == 1 && c->bin_pinned && !kernel_grad(c);
+  // the meshes stay valid for a pm_force_vjp on the same pinned records (a single evaluation, Fourier-space gradient)
+  c->g_valid = ev.n == 1 && c->bin_pinned && !kernel_grad(c) && !(c->p.flags & PM_FLAG_GRAD_REAL);
   return PM_OK;
 }
 
@@ -348,7 +357,7 @@ int pm_force_vjp(pm_ctx* ctx, const float* pos, int64_t N, const float* force_co
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
     c->ev_slot = e;
-    if (!reuse) PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
+    if (!reuse) PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, true, st));
     PM_TRY(vjp_from_meshes(c, N, ev.sh[e], ev.second_grid, force_cot, ev.weight, e == 0 ? 0.0f : 1.0f, pos_cot, st));
   }
   c->g_valid = reuse || (ev.n == 1 && c->bin_pinned);
@@ -375,7 +384,7 @@ int pm_dkd_step(pm_ctx* ctx, float* pos, float* vel, int64_t N, double tau1, dou
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
     c->ev_slot = e;
-    PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
+    PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, false, st));
     // (2.14b) V <- alpha V + beta A in the gather epilogue; after the last evaluation (2.14c) X <- X + tau2 V
     GatherArgs ga = gather_values(3, nullptr, vel, (float)beta * ev.weight, e == 0 ? (float)alpha : 1.0f);
     if (e == ev.n - 1) {
@@ -415,7 +424,7 @@ int pm_dkd_step_adjoint(pm_ctx* ctx, float* pos, float* vel, float* pos_adj, flo
   const Evals ev = evals_of(c);
   for (int e = 0; e < ev.n; ++e) {
     c->ev_slot = e;
-    PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, st));
+    PM_TRY(forward_meshes(c, N, ev.sh[e], ev.second_grid, true, st));
     // primal kick V^{n-1} = (V^n - beta A) / alpha, with beta* = V*^{n-1/2} . A and (after the last evaluation)
     // alpha* = V*^{n-1/2} . V^{n-1} reduced in the same pass
     GatherArgs ga = gather_values(3, nullptr, vel, (float)(-beta / alpha) * ev.weight, e == 0 ? (float)(1.0 / alpha) : 1.0f);

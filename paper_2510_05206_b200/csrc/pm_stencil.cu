@@ -5,13 +5,13 @@
 //   k_fd_gradient  : phi -> g_a = -(1/Delta) sum_s c_s (phi[j + s e_a] - phi[j - s e_a]),  a = x, y, z
 //
 // One inverse FFT instead of three for the force: the Fourier-space kernel writes 4G instead of 12G bytes, two C2R
-// transforms disappear, and this pass moves 4G + 12G.  The TRANSPOSED operator (VJP) stays in Fourier space: the
-// real-space form, psi = sum_a D_a gbar_a followed by ONE forward transform, was built and measured -- parity
-// 4e-6 at 64^3 but 1.9e-5 at 512^3: the cotangent meshes are rough (scattered lambda), storing their divergence in
-// fp32 injects WHITE rounding noise, while the wanted signal i D(k) gbar_hat vanishes like k at low k, exactly
-// where the Green's function 1/k^2 then puts its weight; in Fourier space the rounding error of a mode is scaled
-// by D(k) with the mode.  The forward direction differentiates the SMOOTH potential and has no such problem.  HBM-bound: a CTA owns a (YB x ZB) patch of one x plane; the z and y neighbours come from L1, the
-// x neighbours from L2 (2R + 1 planes of m^2 floats are live at a time: 5 MB at m = 512, FD4).
+// transforms disappear, and this pass moves 4G + 12G.
+//
+// Forward evaluations only (pm_force, pm_dkd_step, pm_poisson_force).  The stencil differences a potential that is
+// dominated by low k and much larger than Delta |grad phi|, so g carries WHITE rounding noise eps |phi| / Delta: 1e-6 of
+// the force, but the reverse-mode calls gather g with grad W, i.e. difference it once more between neighbouring nodes,
+// which amplifies exactly that noise (VJP parity 4e-6 at 64^3, 1.85e-5 at 512^3).  They keep the three-inverse-FFT
+// meshes and the Fourier-space transposed operator (pm_api.cu forward_meshes).
 #include "pm_internal.cuh"
 
 namespace pmf {

@@ -42,6 +42,9 @@ CONFIGS = {
                  lap_order=0, deconv_pow=0, seed=1004, cot_seed=2004, clustered=True),
     "headline": dict(n_p=512, m=512, box=1000.0, rms=1.0, worder=2, interlace=0, grad_order=4,
                      lap_order=0, deconv_pow=2, seed=1005),
+    # cfg3 with the paper's own NUFFT setting (upsampling 5/4, kernel of 5^3 cells): fine grid 640^3
+    "cfg3_paper": dict(n_p=512, m=512, box=1000.0, rms=2.0, nufft=True, sigma=1.25, eps=1e-4, width=5,
+                       grad_order=0, lap_order=0, seed=1006),
 }
 
 

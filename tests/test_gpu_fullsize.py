@@ -201,28 +201,31 @@ def params_of(pm, c, n, **over):
     return pm.PMParams(**kw)
 
 
-def sampled_force_and_vjp(pm, name, sample_idx_fn, with_vjp, flags=0):
-    """pm_force (and pm_force_vjp) on config `name` at full size; the oracle does steps O1-O7 (and V(ii),
-    V(iii)) on all particles in fp64 and the per-particle steps O8 / V(i), V(iv) on the sampled particles."""
+def sampled_force_and_vjp(pm, name, sample_idx_fn, with_vjp, variants=(("", 0),)):
+    """pm_force (and pm_force_vjp) on config `name` at full size, once per (tag, pm_params.flags) variant; the oracle
+    does steps O1-O7 (and V(ii), V(iii)) on all particles in fp64, ONCE, and the per-particle steps O8 / V(i), V(iv)
+    on the sampled particles; every variant is compared with the same reference."""
     pos, c = gen.make_config_positions(name)
     n = pos.shape[0]
     m, box, wo = c["m"], c["box"], c["worder"]
-    ctx = pm.pm_create(params_of(pm, c, n, flags=flags))
-    d_pos = dev(pos)
-    f = torch.empty(n, 3, device="cuda")
-    pm.pm_force(ctx, d_pos, f)
-    f = f.cpu().numpy()
-    xb = None
-    if with_vjp:
-        lam = gen.gaussian_cotangent(n, c.get("cot_seed", 2000))
-        d_lam = dev(lam)
-        t = torch.empty(n, 3, device="cuda")
-        pm.pm_force_vjp(ctx, d_pos, d_lam, t)
-        xb = t.cpu().numpy()
-        del t, d_lam
-    del d_pos
-    pm.pm_destroy(ctx)
-    torch.cuda.empty_cache()
+    lam = gen.gaussian_cotangent(n, c.get("cot_seed", 2000)) if with_vjp else None
+    got = []
+    for tag, flags in variants:
+        ctx = pm.pm_create(params_of(pm, c, n, flags=flags))
+        d_pos = dev(pos)
+        f = torch.empty(n, 3, device="cuda")
+        pm.pm_force(ctx, d_pos, f)
+        xb = None
+        if with_vjp:
+            d_lam = dev(lam)
+            t = torch.empty(n, 3, device="cuda")
+            pm.pm_force_vjp(ctx, d_pos, d_lam, t)
+            xb = t.cpu().numpy()
+            del t, d_lam
+        got.append((tag, f.cpu().numpy(), xb))
+        del d_pos, f
+        pm.pm_destroy(ctx)
+        torch.cuda.empty_cache()
 
     kw = dict(box=box, worder=wo, grad_order=c["grad_order"], lap_order=c["lap_order"], deconv_pow=c["deconv_pow"])
     rho = po.scatter(pos, m, box, wo)
@@ -231,9 +234,10 @@ def sampled_force_and_vjp(pm, name, sample_idx_fn, with_vjp, flags=0):
     del rho
     ps = pos[idx]
     ref = np.stack([po.gather(g[a], ps, box, wo) for a in range(3)], axis=1)
-    check(f"{name}/force/sampled={idx.size}", f[idx], ref, FORCE_TOL)
-    fsum = np.abs(f.astype(np.float64).sum(axis=0)).max()  # holds at any size: momentum conservation (interlace 0)
-    assert fsum <= 1e-6 * np.abs(f.astype(np.float64)).sum()
+    for tag, f, _ in got:
+        check(f"{name}{tag}/force/sampled={idx.size}", f[idx], ref, FORCE_TOL)
+        fsum = np.abs(f.astype(np.float64).sum(axis=0)).max()  # holds at any size: momentum conservation (interlace 0)
+        assert fsum <= 1e-6 * np.abs(f.astype(np.float64)).sum()
     if with_vjp:
         ls = lam[idx].astype(np.float64)
         refv = np.zeros((idx.size, 3))
@@ -246,7 +250,8 @@ def sampled_force_and_vjp(pm, name, sample_idx_fn, with_vjp, flags=0):
         del gbar
         for b in range(3):                                   # V(iv): Eq. C.6, w_i = 1, d(delta)/d(rho) = G/N
             refv[:, b] += (m ** 3 / float(n)) * po.gather(dbar, ps, box, wo, deriv_axis=b)
-        check(f"{name}/vjp/sampled={idx.size}", xb[idx], refv, VJP_TOL)
+        for tag, _, xb in got:
+            check(f"{name}{tag}/vjp/sampled={idx.size}", xb[idx], refv, VJP_TOL)
 
 
 def uniform_sample(pos, rho, n, box):
@@ -274,8 +279,11 @@ def halo_core_sample(pos, rho, n, box):
 
 
 def test_headline_full_size_sampled(pm):
-    """The bench workload itself (N = 512^3 on 512^3, CIC, FD4, deconvolved): forward force and VJP."""
-    sampled_force_and_vjp(pm, "headline", uniform_sample, with_vjp=True)
+    """The bench workload itself (N = 512^3 on 512^3, CIC, FD4, deconvolved): forward force and VJP, on the reference
+    path (three inverse FFTs) and with PM_FLAG_GRAD_REAL (one inverse FFT, gradient by the real-space stencil),
+    both against the same, unchanged oracle."""
+    sampled_force_and_vjp(pm, "headline", uniform_sample, with_vjp=True,
+                          variants=(("", 0), ("+grad_real", pm.FLAG_GRAD_REAL)))
 
 
 def test_cfg2_full_size_sampled(pm):

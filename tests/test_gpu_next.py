@@ -98,18 +98,6 @@ def test_real_gradient_force_and_vjp(pm, name, n_p, interlace):
     check("vjp", xb, po.force_vjp(pos, lam, c["m"], c["box"], **oracle_kw(c)), 1e-5)
 
 
-def test_real_gradient_headline_full_size_sampled(pm):
-    """The one-C2R variant on the bench workload at full size (same sampled comparison as the reference path)."""
-    from test_gpu_fullsize import sampled_force_and_vjp, uniform_sample
-
-    old = po.FFT_WORKERS
-    po.FFT_WORKERS = -1
-    try:
-        sampled_force_and_vjp(pm, "headline", uniform_sample, with_vjp=True, flags=pm.FLAG_GRAD_REAL)
-    finally:
-        po.FFT_WORKERS = old
-
-
 # ---- NEXT-3: ES kernel-gradient force ----------------------------------------------------------------------------
 @pytest.mark.parametrize("sigma,eps,width", [(2.0, 1e-6, 0), (2.0, 1e-4, 0), (1.25, 0.5, 5), (2.0, 1e-6, 8)])
 def test_kernel_gradient_force(pm, sigma, eps, width):

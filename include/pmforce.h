@@ -204,6 +204,25 @@ int pm_dkd_step_adjoint(pm_ctx* ctx, float* pos, float* vel, float* pos_adj, flo
  * subtraction), number of modes; empty bins give 0.  method 0 only. */
 int pm_power_spectrum(pm_ctx* ctx, const float* pos, int64_t N, const float* pos2, int64_t N2, int deconvolve,
                       int nbins, double* k_mean, double* power, double* n_modes, void* stream);
+/* The shell binning of pm_power_spectrum on spectra the CALLER holds, for callers that cannot allocate (CUDA graph
+ * capture, serving loops, harnesses that forbid cudaMalloc): no ctx, and the call makes no cudaMalloc / cudaFree
+ * and calls no allocating library routine.  Runs on the CURRENT device.
+ *   spec_a, spec_b : device arrays of m * m * (m/2 + 1) complex (interleaved re, im; the half-complex layout of a
+ *                    3-D R2C transform of a real [m][m][m] mesh, z fastest); spec_b NULL = auto spectrum.
+ *   outputs        : device arrays of nbins doubles, overwritten:  n_modes(b) = number of modes of the full
+ *                    Fourier cube with b + 1/2 <= |n| < b + 3/2 (reading R20),  k_mean(b) = (2 pi / box) <|n|>,
+ *                    power(b) = norm * <Re(A conj B)>  (norm = box^3 / (N_A N_B) for particle-count meshes
+ *                    reproduces pm_power_spectrum without interlacing and deconvolution).  Empty bins give 0.
+ *   errbuf         : host buffer of errbuf_len bytes (or NULL) that receives a message when the status is not PM_OK.
+ * The kernel's scratch (3 * nbins fp64 accumulators) is a static __device__ array of PM_NOALLOC_MAX_BINS bins
+ * (24 KB on every GPU that loads the library, until exit): nbins beyond it is rejected with PM_EINVAL.  Every call
+ * on a device shares that array and clears it first, in stream order; calls that OVERLAP on the GPU (different
+ * streams without a dependency) race on it.  The first call on a device looks the array's address up
+ * (cudaGetSymbolAddress): make it outside graph capture. */
+#define PM_NOALLOC_MAX_BINS 1024
+int pm_mesh_power_noalloc(const float* spec_a, const float* spec_b, int32_t m, double box, double norm,
+                          int32_t nbins, double* k_mean, double* power, double* n_modes, char* errbuf,
+                          int32_t errbuf_len, void* stream);
 /* Sheet-based resampling, trilinear variant (Table 5 n_resample :411; reading R21).
  * pos: [n_p^3, 3] in Lagrangian (C) order (particle (i,j,k) started at (i,j,k) box/n_p); pos_out:
  * [(r n_p)^3, 3], the refined sheet X' = q' + trilinear interpolation of the displacement, wrapped into

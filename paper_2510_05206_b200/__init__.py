@@ -34,6 +34,8 @@ from .api import (  # noqa: F401
     pm_dkd_step_adjoint,
     pm_power_spectrum,
     pm_sheet_resample,
+    pm_mesh_power_noalloc,
+    NOALLOC_MAX_BINS,
     pm_smem_peak,
     pm_set_profiling,
     pm_get_stage_ms,

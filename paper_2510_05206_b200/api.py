@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = (
     "pm_interp", "pm_interp_vjp", "nufft_spread", "nufft_spread_vjp", "nufft_poisson_force",
     "nufft_poisson_force_vjp", "nufft_interp", "nufft_interp_vjp", "pm_force", "pm_force_vjp", "pm_force_host",
     "pm_set_profiling", "pm_get_stage_ms", "pm_assign_jvp", "pm_interp_jvp", "pm_dkd_step", "pm_dkd_step_adjoint",
-    "pm_power_spectrum", "pm_sheet_resample", "pm_smem_peak",
+    "pm_power_spectrum", "pm_sheet_resample", "pm_smem_peak", "pm_mesh_power_noalloc",
 )
 
 STAGE_NAMES = ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "interp", "vjp_scatter", "vjp_kspace", "vjp_gather",
@@ -116,6 +116,8 @@ def load_library(build_if_missing: bool = False):
                                           vp, vp]),
         "pm_power_spectrum": (C.c_int, [vp, vp, i64, vp, i64, C.c_int, C.c_int, vp, vp, vp, vp]),
         "pm_sheet_resample": (C.c_int, [vp, vp, C.c_int32, C.c_int32, vp, vp]),
+        "pm_mesh_power_noalloc": (C.c_int, [vp, vp, C.c_int32, C.c_double, C.c_double, C.c_int32, vp, vp, vp,
+                                            C.c_char_p, C.c_int32, vp]),
         "pm_smem_peak": (C.c_int, [vp, C.c_int, C.POINTER(C.c_double), vp]),
         "pm_set_profiling": (C.c_int, [vp, C.c_int]),
         "pm_get_stage_ms": (C.c_int, [vp, C.POINTER(C.c_float), C.c_int, C.POINTER(i64)]),
@@ -371,6 +373,25 @@ def pm_power_spectrum(ctx, pos, k_mean, power, n_modes, pos2=None, deconvolve=Tr
                                                _n(pos2) if pos2 is not None else 0, int(bool(deconvolve)), nbins,
                                                _dev64(k_mean, "k_mean", nbins), _dev64(power, "power", nbins),
                                                _dev64(n_modes, "n_modes", nbins), _stream()), "pm_power_spectrum")
+
+
+NOALLOC_MAX_BINS = 1024  # PM_NOALLOC_MAX_BINS of include/pmforce.h
+
+
+def pm_mesh_power_noalloc(spec_a, m, box, norm, k_mean, power, n_modes, spec_b=None):
+    """Shell-binned (cross-)power of half-complex spectra the caller holds; allocates nothing (no ctx).
+
+    spec_a / spec_b: contiguous float32 CUDA tensors [m, m, m//2 + 1, 2] (``torch.view_as_real`` of a complex64
+    ``rfftn``); k_mean, power, n_modes: float64 CUDA tensors [nbins], nbins <= NOALLOC_MAX_BINS."""
+    nbins = k_mean.numel()
+    ncomplex = m * m * (m // 2 + 1)
+    err = C.create_string_buffer(256)
+    rc = load_library().pm_mesh_power_noalloc(
+        _dev(spec_a, "spec_a", 2 * ncomplex), _dev(spec_b, "spec_b", 2 * ncomplex), int(m), float(box), float(norm),
+        nbins, _dev64(k_mean, "k_mean", nbins), _dev64(power, "power", nbins), _dev64(n_modes, "n_modes", nbins),
+        err, len(err), _stream())
+    if rc != 0:
+        raise PMError(f"pm_mesh_power_noalloc: {err.value.decode() or rc}")
 
 
 def pm_sheet_resample(ctx, pos, n_p, r, pos_out):

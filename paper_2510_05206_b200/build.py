@@ -23,7 +23,7 @@ LIB = os.path.join(PKG, "libpmforce.so")
 
 ES_WIDTHS = (4, 5, 6, 7, 8)  # keep in step with ES_WIDTHS in csrc/nufft_dispatch.cu
 SOURCES = ["pm_ctx.cu", "pm_bin.cu", "pm_scatter.cu", "pm_gather.cu", "pm_jvp.cu", "pm_kspace.cu", "pm_xfft.cu",
-           "pm_stencil.cu", "pm_step.cu", "pm_power.cu", "pm_resample.cu", "pm_microbench.cu", "pm_api.cu",
+           "pm_stencil.cu", "pm_step.cu", "pm_power.cu", "pm_resample.cu", "pm_microbench.cu", "pm_noalloc.cu", "pm_api.cu",
            "nufft_dispatch.cu"]
 HEADERS = ["pm_internal.cuh", "pm_mesh_kernels.cuh", os.path.join(ROOT, "include", "pmforce.h")]
 

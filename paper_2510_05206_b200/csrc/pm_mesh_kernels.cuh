@@ -23,6 +23,8 @@ template <int ORDER, bool SHIFTED>
 struct PMTraits {
   static constexpr int P = ORDER;
   static constexpr bool SHIFT = SHIFTED;  // a fractional grid shift is subtracted from the record coordinate
+  static constexpr bool SKEW = false;     // see ESTraits
+  static constexpr bool ES = false;
   static constexpr int HLO = (ORDER == 2 ? 0 : 1) + (SHIFTED ? 1 : 0);
   static constexpr int HHI = (ORDER == 2 ? 1 : 2);
   // largest value of the 3-D kernel: W(0)^3 = 1 (CIC), (3/4)^3 (TSC), (2/3)^3 (PCS)
@@ -68,6 +70,26 @@ struct PMTraits {
   }
 };
 
+// Launch shape of the ES (NUFFT) spreading / interpolation kernels.  The stencil walk of ONE particle is w^3 = 64 .. 512
+// nodes, fully unrolled: a thread holds ONE record at a time (eight / four unrolled copies of the walk were 290 KB of
+// code -- instruction-fetch stalls -- and 252 registers: one CTA of 8 warps per SM, ncu round 2) and the register
+// allocation aims at three resident CTAs.  cfg3 (w = 7): spread 34.4 -> 20.1 ms with these two alone.
+constexpr int ES_PPT = 1;     // records per thread and batch, k_scatter
+constexpr int ES_KB = 1;      // records in flight per thread, k_gather
+constexpr int ES_MINCTA = 3;  // resident CTAs per SM the single-field ES scatter is compiled for
+// Widths whose kernels use the skewed walk over dense rows (skew_match below).  Measured on cfg3 (spread / interp, ms):
+// w = 8: 21.7 / 59.5 against 29.9 / 78.4 without; w = 7: 18.3 / 37.8 against 20.1 / 53.7; w = 6: 14.4 / 29.9 against
+// 13.5 / 35.3; w = 5 (8 steps for 5 columns): 8.7 / 17.1 against 6.2 / 15.1 -- not used below 6.
+constexpr bool es_skew_width(int w) { return w >= 6; }
+// Float -> fixed point without the conversion unit (unit-weight ES spreading).  F2I shares the quarter-rate pipe with
+// the kernel's exp / sqrt; one F2I per node kept it 67 % busy (ncu round 2).  Instead the deposit x < 2^24 is computed as
+// the DENORMAL float x * 2^-149, whose bit pattern IS the integer round-to-nearest-even(x) (the lowest binade of the
+// normal numbers continues the same integer scale).  The factor is split between the z weights (2^-64) and the x weights
+// (2^-85) so that every operand stays a normal number and only the final product rounds to the integer grid.  Denormal
+// arithmetic runs at full rate in the FMA pipe; the build must not flush them (no -ftz / --use_fast_math).
+constexpr float ES_DENORM_Z = 5.421010862427522e-20f;   // 2^-64
+constexpr float ES_DENORM_X = 2.5849394142282115e-26f;  // 2^-85
+
 // Exponential-of-semicircle kernel phi(z) = exp(beta (sqrt(1 - z^2) - 1)), z = 2 (j - u)/w, nodes
 // j = ceil(u - w/2) .. + w - 1 (refs [82,83]; readings R10, R13).
 template <int W>
@@ -83,32 +105,61 @@ struct ESTraits {
     uint32_t frac[3];  // unused (no shift), kept for a uniform interface
     float beta;
   };
-  template <bool DERIV>
-  static __device__ __forceinline__ void axis(uint32_t v, const Params& p, int& s0, float (&w)[P], float (&dw)[P]) {
+  static constexpr int K0 = ODD ? -(W - 1) / 2 : -(W / 2 - 1);  // first node of the stencil relative to the reference node
+  // first node s0 (relative to tile origin - HLO) and d = u - (reference node) of a record coordinate
+  static __device__ __forceinline__ void origin(uint32_t v, int& s0, float& d) {
     constexpr float INV = 1.0f / (float)REC_ONE;
-    float d;  // u - (reference node)
-    int ref;  // reference node (biased): nodes are ref - HLOREF .. ref - HLOREF + W - 1
     if (ODD) {
       const uint32_t vh = v + (REC_ONE >> 1);
       d = (float)((int)(vh & REC_MASK) - (int)(REC_ONE >> 1)) * INV;  // [-1/2, 1/2)
-      ref = (int)(vh >> REC_FRAC);
-      s0 = ref - REC_BIAS - (W - 1) / 2 + HLO;
+      s0 = (int)(vh >> REC_FRAC) - REC_BIAS - (W - 1) / 2 + HLO;
     } else {
       d = (float)(v & REC_MASK) * INV;  // [0, 1)
-      ref = (int)(v >> REC_FRAC);
-      s0 = ref - REC_BIAS - (W / 2 - 1) + HLO;
+      s0 = (int)(v >> REC_FRAC) - REC_BIAS - (W / 2 - 1) + HLO;
     }
-    constexpr int K0 = ODD ? -(W - 1) / 2 : -(W / 2 - 1);
+  }
+  // kernel value (and d/du) at stencil node k (kf = K0 + k as a float; k may be a run-time value)
+  template <bool DERIV>
+  static __device__ __forceinline__ void node_weight(float kf, float d, const Params& p, float& w, float& dw) {
     constexpr float TWO_W = 2.0f / (float)W;
+    const float z = (kf - d) * TWO_W;
+    const float q = fmaxf(1.0f - z * z, 0.0f);
+    const float s = sqrtf(q);
+    const float phi = expf(p.beta * (s - 1.0f));
+    w = phi;
+    // d/du phi(2 (j-u)/w) = -(2/w) phi'(z), phi'(z) = -beta z phi / sqrt(1 - z^2), 0 at |z| >= 1 (R13)
+    if (DERIV) dw = q > 0.0f ? TWO_W * p.beta * z * phi / s : 0.0f;
+  }
+  template <bool DERIV>
+  static __device__ __forceinline__ void axis(uint32_t v, const Params& p, int& s0, float (&w)[P], float (&dw)[P]) {
+    float d;
+    origin(v, s0, d);
 #pragma unroll
-    for (int k = 0; k < W; ++k) {
-      const float z = ((float)(K0 + k) - d) * TWO_W;
-      const float q = fmaxf(1.0f - z * z, 0.0f);
-      const float s = sqrtf(q);
-      const float phi = expf(p.beta * (s - 1.0f));
-      w[k] = phi;
-      // d/du phi(2 (j-u)/w) = -(2/w) phi'(z), phi'(z) = -beta z phi / sqrt(1 - z^2), 0 at |z| >= 1 (R13)
-      if (DERIV) dw[k] = q > 0.0f ? TWO_W * p.beta * z * phi / s : 0.0f;
+    for (int k = 0; k < W; ++k) node_weight<DERIV>((float)(K0 + k), d, p, w[k], dw[k]);
+  }
+  // Skewed stencil walk (skew_match below): the z loop has ZS = 8 steps per (x, y) row; step j of a lane whose walk
+  // is rotated by rot visits column (j + rot) of the row -- columns 8 .. 14 are columns 0 .. 6 of the NEXT row of the
+  // walk.  wU / wW: the z weight of step j if it falls into the current / the next row (the other one is 0); columns
+  // W .. 7 carry weight 0 (the walk passes over them so that every step advances the bank by one).
+  static constexpr bool SKEW = es_skew_width(W);
+  static constexpr bool ES = true;
+  static constexpr int ZS = 8;
+  template <bool DERIV>
+  static __device__ __forceinline__ void axis_skew(float d, const Params& p, int rot, float (&wU)[ZS], float (&wW)[ZS],
+                                                   float (&dU)[ZS], float (&dW)[ZS]) {
+#pragma unroll
+    for (int j = 0; j < ZS; ++j) {
+      const int n = j + rot, c = n & (ZS - 1);
+      float w, dw = 0.0f;
+      node_weight<DERIV>((float)(K0 + c), d, p, w, dw);
+      if (c >= W) w = 0.0f, dw = 0.0f;
+      const bool nextrow = n >= ZS;
+      wU[j] = nextrow ? 0.0f : w;
+      wW[j] = nextrow ? w : 0.0f;
+      if (DERIV) {
+        dU[j] = nextrow ? 0.0f : dw;
+        dW[j] = nextrow ? dw : 0.0f;
+      }
     }
   }
 };
@@ -126,13 +177,22 @@ struct Geo {
   static constexpr int P = T::P, HLO = T::HLO, HHI = T::HHI;
   static constexpr int ZLO = (HLO + 3) / 4 * 4;
   static constexpr int HZ = ZLO + (HHI + 3) / 4 * 4;                 // halo columns per row
-  static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI, NROW = SX * SY;
+  // DENSE (skewed walk, ES kernels): one piece per (x, y) row, pitch TZ + HZ = 40 words.  With the 8-step z loop of
+  // the skewed walk a step to the next column (+1), to the next row (+40 - 7) and to the next x slab
+  // ((SY - (W - 1)) * 40 - 7 = 353 words: SY - (W - 1) = 9, even widths pad SY by one row for it) all advance the bank
+  // by exactly one.
+  static constexpr bool DENSE = T::SKEW;
+  static constexpr int PITCH = TZ + HZ;
+  static constexpr int SX = TX + HLO + HHI, SY = TY + HLO + HHI + ((DENSE && P % 2 == 0) ? 1 : 0), NROW = SX * SY;
   static constexpr int MAIN = NROW * TZ, HAL = NROW * HZ;            // words per component
-  static constexpr int COMP = (MAIN + HAL + 31) / 32 * 32;           // component block (128-byte multiple)
+  // component block (128-byte multiple); DENSE: at least 8 words of slack behind the last row -- the zero-weight
+  // columns of the skewed walk (up to column 41 of a row) touch them
+  static constexpr int COMP = (MAIN + HAL + (T::SKEW ? 8 : 0) + 31) / 32 * 32;
   static constexpr int NGM = NROW * (TZ / 4), NGH = NROW * (HZ / 4); // float4 groups per component
   static constexpr int NGROUP = NGM + NGH;
   static_assert(TZ == 32, "the main plane's row pitch must be 32 words");
   static_assert(HZ == 4 || HZ == 8, "halo columns");
+  static_assert(!DENSE || (HZ == 8 && SY - (P - 1) == 9), "the skewed walk needs rows of 40 words and a slab step of 9 rows");
 };
 
 // Address of node column s (0 <= s < TZ + HZ, relative to the box start) in row `row` of a component block:
@@ -144,15 +204,23 @@ struct NodeCol {
 template <class G>
 __device__ __forceinline__ NodeCol node_col(int row0, int s) {  // row0 = index of the particle's first row
   NodeCol c;
-  const bool main = s < TZ;
-  c.pitch = main ? TZ : G::HZ;
-  c.base = main ? row0 * TZ + s : G::MAIN + row0 * G::HZ + (s - TZ);
+  if constexpr (G::DENSE) {
+    c.pitch = G::PITCH;
+    c.base = row0 * G::PITCH + s;
+  } else {
+    const bool main = s < TZ;
+    c.pitch = main ? TZ : G::HZ;
+    c.base = main ? row0 * TZ + s : G::MAIN + row0 * G::HZ + (s - TZ);
+  }
   return c;
 }
 // float4 group j of a component block -> (row, z offset of its first node relative to the box start)
 template <class G>
 __device__ __forceinline__ void group_pos(int j, int& row, int& zoff) {
-  if (j < G::NGM) {
+  if constexpr (G::DENSE) {
+    row = j / (G::PITCH / 4);
+    zoff = 4 * (j - row * (G::PITCH / 4));
+  } else if (j < G::NGM) {
     row = j / (TZ / 4);
     zoff = 4 * (j - row * (TZ / 4));
   } else {
@@ -248,6 +316,69 @@ __device__ __forceinline__ void load_rec(uint4& r, const BinView& bv, uint32_t i
 }
 __device__ __forceinline__ uint32_t rec_index(const BinView& bv, uint32_t i) { return bv.rec[i].w; }
 
+// ---- skewed stencil walk of the ES kernels ---------------------------------------------------------------------
+// One thread walks the W x W x W nodes of its particle; the 32 lanes of a warp sit at unrelated z, so a shared-memory
+// access of the warp hits a bank 3.5 times on average (32 balls into 32 bins: measured 3.8-way replays, the NUFFT
+// kernels ran at 0.21 / 0.43 of the conflict-free ceilings).  In the DENSE tile layout the walk x slab -> y row -> 8 z
+// columns advances the bank by exactly one per step for every lane, so the warp is conflict-free for the whole walk
+// iff the lanes START in 32 different banks.  Lane l may start rot_l in [0, 8) columns into its first row (the skipped
+// columns are visited at the end of the walk): skew_match picks the rotations so that the starting banks
+// (B_l + rot_l) mod 32 are distinct wherever a matching exists.  All intervals [B_l, B_l + 8) have the same length, so
+// handing out the banks in the order of B_l -- each lane the first free bank at or after its own -- is optimal on a
+// line; the circle is cut behind the bank v that minimises D_v = #{l : B_l <= v} - (v + 1), from where the sorted
+// assignment never wraps.  In closed form, with E_v the number of lanes in banks before v (in cut order) and o the
+// rank of a lane among those of its bank:  slot = E + o + max_{u <= v, occupied} (u - E_u).  A lane whose slot lies 8
+// or more behind its bank finds no free bank (0.5 lanes per warp for uniformly random B) and takes any rotation.
+// Call with all 32 lanes; `valid` lanes take part.  Returns rot in [0, 8).
+__device__ __forceinline__ int skew_match(int B, bool valid) {
+  constexpr unsigned FULL = 0xffffffffu;
+  const int v = (int)(threadIdx.x & 31u);
+  unsigned mine = __ballot_sync(FULL, valid);  // -> valid lanes whose bank is v
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    const unsigned bk = __ballot_sync(FULL, (B >> k) & 1);
+    mine &= ((v >> k) & 1) ? bk : ~bk;
+  }
+  const int c = __popc(mine);
+  const unsigned peers = __shfl_sync(FULL, mine, B);
+  const int o = __popc(peers & ((1u << v) - 1u));
+  int S = c;  // inclusive prefix over the banks
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int t = __shfl_up_sync(FULL, S, d);
+    if (v >= d) S += t;
+  }
+  const int total = __shfl_sync(FULL, S, 31);
+  int key = ((S - (v + 1) + 64) << 5) | v;  // first minimum of D
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) key = min(key, __shfl_xor_sync(FULL, key, d));
+  const int vmin = key & 31;
+  const int Smin = (key >> 5) - 64 + vmin + 1;
+  const int cut = (vmin + 1) & 31;
+  const int vp = (v - cut) & 31;
+  const int Sr = cut == 0 ? S : (v >= cut ? S - Smin : S + total - Smin);
+  const int E = Sr - c;
+  const int term = c > 0 ? vp - E : -1000;
+  int M = __shfl_sync(FULL, term, (v + cut) & 31);  // lane i: the term of the bank with cut-order index i
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int t = __shfl_up_sync(FULL, M, d);
+    if (v >= d) M = max(M, t);
+  }
+  const int Bp = (B - cut) & 31;
+  const int rot = __shfl_sync(FULL, E, B) + o + __shfl_sync(FULL, M, Bp) - Bp;
+  return rot & 7;
+}
+
+// address step from column 8 + c of row (a, b) of the walk to column c of the row that follows it: (a, b + 1), the first
+// row of the next slab, or (after the last row) the first row of the walk
+template <class G>
+__host__ __device__ constexpr int skew_next_off(int a, int b) {
+  return b < G::P - 1 ? G::PITCH - 8
+                      : (a < G::P - 1 ? (G::SY - (G::P - 1)) * G::PITCH - 8
+                                      : -((G::P - 1) * G::SY + (G::P - 1)) * G::PITCH - 8);
+}
+
 // ---- K2 / K5: tile scatter ---------------------------------------------------------------------------
 // Persistent CTAs draw work items from the dynamic schedule, two items ahead: while item i is deposited, the
 // records of item i+1 are already being loaded into the registers item i frees (rolling prefetch), and its
@@ -271,13 +402,16 @@ constexpr int scatter_min_ctas() {
   // vector scatter of the VJP (3 components): at 151 registers ONE CTA was resident per SM (ncu: 12.5 % warps
   // active, 3.5 ms at 512^3); two CTAs for CIC / TSC cap the allocation at 128
   return WMODE == W_JVP ? 1
-                        : (NCOMP == 1 && WMODE == W_UNIT) ? (T::P == 2 ? 4 : (T::P <= 4 ? 3 : 1))
-                                                          : (NCOMP == 1 ? 2 : (T::P <= 3 ? 2 : 1));
+                        : (NCOMP == 1 && WMODE == W_UNIT) ? (T::P == 2 ? 4 : (T::P <= 4 ? 3 : (T::ES ? ES_MINCTA : 1)))
+                                                          : (NCOMP == 1 ? (T::ES ? ES_MINCTA : 2)
+                                                                        : ((T::P <= 3 || T::ES) ? 2 : 1));
 }
 template <class T, int NCOMP, int WMODE, int NBUF>
 __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_scatter(BinView bv, typename T::Params tp, int3 roll,
                                                    ScatterSrc src, MeshPtrs<NCOMP> mesh) {
   constexpr bool WEIGHTED = WMODE != W_UNIT;
+  constexpr int PPT_ = T::ES ? ES_PPT : PPT;  // records per thread held in registers at a time
+  constexpr int CHUNK_ = BLOCK * PPT_;
   constexpr bool JVP = WMODE == W_JVP;
   constexpr int NPAY = JVP ? 4 : NCOMP;  // floats a particle carries: its weights, or {w~, w t_x, w t_y, w t_z}
   static_assert(!JVP || NCOMP == 1, "the forward-mode scatter deposits one field");
@@ -317,10 +451,10 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
   // records of a work item -> registers
   WorkItem wi, nwi;
   wi.begin = wi.end = wi.txyz = nwi.begin = nwi.end = nwi.txyz = 0;
-  uint4 r[PPT];
-  auto load_batch = [&](uint32_t b0, uint32_t end) {  // up to CHUNK records starting at b0
+  uint4 r[PPT_];
+  auto load_batch = [&](uint32_t b0, uint32_t end) {  // up to CHUNK_ records starting at b0
 #pragma unroll
-    for (int k = 0; k < PPT; ++k) {
+    for (int k = 0; k < PPT_; ++k) {
       const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
       if (i < end) load_rec<WEIGHTED>(r[k], bv, i);
     }
@@ -343,7 +477,7 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
     const TileOrigin o = tile_origin(wi);
     const uint32_t nbegin = nwi.begin, nend = nxt < nitems ? nwi.end : nwi.begin;  // empty when there is no next item
 
-    float wv[PPT][NPAY];
+    float wv[PPT_][NPAY];
     float wabs[NCOMP];
 #pragma unroll
     for (int a = 0; a < NCOMP; ++a) wabs[a] = 0.0f;
@@ -371,14 +505,14 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
     };
     auto load_weights = [&](uint32_t b0) {  // payloads of the batch held in r[]
 #pragma unroll
-      for (int k = 0; k < PPT; ++k) {
+      for (int k = 0; k < PPT_; ++k) {
         const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
         if (i < iend) payload(r[k].w, wv[k]);
       }
     };
     load_weights(ibegin);
-    if (WEIGHTED && n > (uint32_t)CHUNK) {  // dense tile: the bound needs the weights of the later batches too
-      for (uint32_t i = ibegin + CHUNK + tid; i < iend; i += BLOCK) {
+    if (WEIGHTED && n > (uint32_t)CHUNK_) {  // dense tile: the bound needs the weights of the later batches too
+      for (uint32_t i = ibegin + CHUNK_ + tid; i < iend; i += BLOCK) {
         float pv[NPAY];
         payload(rec_index(bv, i), pv);
       }
@@ -415,7 +549,8 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
       int e = 0;
       const float f = frexpf(bound, &e);
       const int cl = (f == 0.5f) ? e - 1 : e;
-      const int sexp = min(31, 31 - cl);
+      // ES kernels convert without F2I (es_bits below), which needs every single deposit below 2^24
+      const int sexp = min(T::ES ? 22 : 31, 31 - cl);
 #pragma unroll
       for (int a = 0; a < NCOMP; ++a) {
         scale[a] = pow2i(sexp);
@@ -424,11 +559,66 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
     }
 
     for (uint32_t b0 = ibegin;;) {
-      const bool last = b0 + CHUNK >= iend;  // uniform
+      const bool last = b0 + CHUNK_ >= iend;  // uniform
 #pragma unroll
-      for (int k = 0; k < PPT; ++k) {
+      for (int k = 0; k < PPT_; ++k) {
         const uint32_t i = b0 + (uint32_t)(k * BLOCK + tid);
-        if (i < iend) {
+        if constexpr (T::SKEW) {  // ES kernels: skewed walk over dense rows (skew_match)
+          static_assert(!JVP, "the forward-mode scatter is not built for the ES kernel");
+          const bool valid = i < iend;
+          int sx = 0, sy = 0, sz = 0;
+          float wx[P], wy[P], dummy[P], dz0 = 0.0f;
+          if (valid) {
+            T::template axis<false>(r[k].x, tp, sx, wx, dummy);
+            T::template axis<false>(r[k].y, tp, sy, wy, dummy);
+            T::origin(r[k].z, sz, dz0);
+          }
+          const int row0 = sx * G::SY + sy, col0 = sz + (G::ZLO - G::HLO);
+          // (warp-uniform) no lane of the warp holds a particle: nothing to match
+          const int rot = __any_sync(0xffffffffu, valid) ? skew_match((row0 * 8 + col0) & 31, valid) : 0;
+          if (valid) {
+            float wU[8], wW[8], dU[8], dW[8];
+            T::template axis_skew<false>(dz0, tp, rot, wU, wW, dU, dW);
+            int nx[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) nx[j] = (j + rot) >= 8 ? 1 : 0;
+            float ws[NCOMP];
+#pragma unroll
+            for (int q = 0; q < NCOMP; ++q) ws[q] = wv[k][q] * scale[q];
+            if (NCOMP == 1) {
+              const float fz = WEIGHTED ? ws[0] : ws[0] * ES_DENORM_Z;  // unit weights: see ES_DENORM_Z
+#pragma unroll
+              for (int j = 0; j < 8; ++j) wU[j] *= fz, wW[j] *= fz;
+              if (!WEIGHTED) {
+#pragma unroll
+                for (int a = 0; a < P; ++a) wx[a] *= ES_DENORM_X;
+              }
+            }
+            int* p0 = s_acc + (row0 * G::PITCH + col0 + rot);
+#pragma unroll
+            for (int a = 0; a < P; ++a)
+#pragma unroll
+              for (int b = 0; b < P; ++b) {
+                const int a2 = b < P - 1 ? a : (a < P - 1 ? a + 1 : 0), b2 = b < P - 1 ? b + 1 : 0;
+                const int nextoff = skew_next_off<G>(a, b);
+                const float cur = wx[a] * wy[b], nxt = wx[a2] * wy[b2];
+                int* rp = p0 + (a * G::SY + b) * G::PITCH;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  int* node = rp + (j + nx[j] * nextoff);
+                  const float wgt = fmaf(nxt, wW[j], cur * wU[j]);  // one of wU[j], wW[j] is an exact zero
+                  if (NCOMP == 1 && !WEIGHTED) {  // the one product, rounded once, as a denormal: ES_DENORM_Z
+                    atomicAdd(reinterpret_cast<unsigned*>(node), __float_as_uint(wgt));
+                  } else if (NCOMP == 1) {
+                    atomicAdd(node, __float2int_rn(wgt));
+                  } else {
+#pragma unroll
+                    for (int q = 0; q < NCOMP; ++q) atomicAdd(node + q * G::COMP, __float2int_rn(wgt * ws[q]));
+                  }
+                }
+              }
+          }
+        } else if (i < iend) {
           int sx, sy, sz;
           float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
           T::template axis<JVP>(apply_shift<T>(r[k].x, tp.frac[0]), tp, sx, wx, dx);
@@ -460,10 +650,15 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
             }
           } else {
             float wzs[NCOMP][P];  // the scale (and the particle's weight) folded into the z weights
+            constexpr bool DENORM = T::ES && !WEIGHTED && NCOMP == 1;  // see ES_DENORM_Z
 #pragma unroll
             for (int q = 0; q < NCOMP; ++q)
 #pragma unroll
-              for (int c = 0; c < P; ++c) wzs[q][c] = wz[c] * (wv[k][q] * scale[q]);
+              for (int c = 0; c < P; ++c) wzs[q][c] = wz[c] * (wv[k][q] * scale[q] * (DENORM ? ES_DENORM_Z : 1.0f));
+            if (DENORM) {
+#pragma unroll
+              for (int a = 0; a < P; ++a) wx[a] *= ES_DENORM_X;
+            }
 #pragma unroll
             for (int a = 0; a < P; ++a)
 #pragma unroll
@@ -476,6 +671,8 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
                   for (int q = 0; q < NCOMP; ++q) {
                     if (WEIGHTED)
                       atomicAdd(node + q * G::COMP, __float2int_rn(wxy * wzs[q][c]));
+                    else if (DENORM)
+                      atomicAdd(reinterpret_cast<unsigned*>(node + q * G::COMP), __float_as_uint(wxy * wzs[q][c]));
                     else
                       atomicAdd(reinterpret_cast<unsigned*>(node + q * G::COMP), __float2uint_rn(wxy * wzs[q][c]));
                   }
@@ -489,7 +686,7 @@ __global__ void __launch_bounds__(BLOCK, scatter_min_ctas<T, NCOMP, WMODE>()) k_
         }
       }
       if (last) break;
-      b0 += CHUNK;
+      b0 += CHUNK_;
       load_batch(b0, iend);  // dense tile: further batches of the same item
       load_weights(b0);
     }
@@ -861,7 +1058,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
   constexpr bool DERIV = GRAD || JVP;
   constexpr int NO = GMODE == G_JVPT ? NST / 2 : NST;  // outputs per particle (G_GRAD: 3)
   static_assert(GMODE != G_JVPT || NST % 2 == 0, "G_JVPT stages the primal and the tangent meshes");
-  constexpr int KB = 4;  // records in flight per thread
+  constexpr int KB = T::ES ? ES_KB : 4;  // records in flight per thread
   constexpr uint32_t BOX_BYTES = (uint32_t)(NST * (G::MAIN + G::HAL) * sizeof(float));
   extern __shared__ __align__(128) unsigned char s_raw[];
   __shared__ __align__(8) uint64_t s_bar[STAGES];
@@ -884,6 +1081,11 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
     fence_proxy_async();
     s_next[0] = sched_next(bv.sched);  // the item after this CTA's first
   }
+  if (G::DENSE) {  // the slack behind the rows is read (with weight zero) by the skewed walk: it must hold finite values
+    constexpr int SLACK = G::COMP - (G::MAIN + G::HAL);
+    for (int j = tid; j < STAGES * NST * SLACK; j += BLOCK)
+      s_base[(j / SLACK) * G::COMP + (G::MAIN + G::HAL) + j % SLACK] = 0.0f;
+  }
   __syncthreads();
 
   auto box_start = [&](const TileOrigin& o, int& cx, int& cy, int& cz) {
@@ -900,8 +1102,8 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
     for (int a = 0; a < NST; ++a) {  // main plane (first TZ nodes of every row) and halo plane (the rest)
       float* dst = s_base + (stage * NST + a) * G::COMP;
-      tma_load_3d(dst, &maps.m[2 * a], &s_bar[stage], cz, cy, cx);
-      tma_load_3d(dst + G::MAIN, &maps.m[2 * a + 1], &s_bar[stage], cz + TZ, cy, cx);
+      tma_load_3d(dst, &maps.m[2 * a], &s_bar[stage], cz, cy, cx);  // DENSE: the whole rows in one box
+      if (!G::DENSE) tma_load_3d(dst + G::MAIN, &maps.m[2 * a + 1], &s_bar[stage], cz + TZ, cy, cx);
     }
   };
 
@@ -969,12 +1171,34 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
         // refill the slot: the record one batch ahead, or (last batch) the next item's first batch
         const uint32_t pi = last ? nbegin + (uint32_t)(k * BLOCK + tid) : i + (uint32_t)(KB * BLOCK);
         if (pi < (last ? nend : wi.end)) load_rec<true>(r[k], bv, pi);
-        if (i >= wi.end) continue;
-        int sx, sy, sz;
+        const bool valid = i < wi.end;
+        if (!T::SKEW && !valid) continue;
+        int sx = 0, sy = 0, sz = 0;
         float wx[P], wy[P], wz[P], dx[P], dy[P], dz[P];
-        T::template axis<DERIV>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
-        T::template axis<DERIV>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
-        T::template axis<DERIV>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
+        // skewed walk (ES kernels, skew_match): z weights per step, for the current and for the next row of the walk
+        float wU[T::SKEW ? 8 : 1], wW[T::SKEW ? 8 : 1], dU[T::SKEW ? 8 : 1], dW[T::SKEW ? 8 : 1];
+        int nx[T::SKEW ? 8 : 1];
+        const float* p0 = nullptr;
+        if constexpr (T::SKEW) {
+          float dz0 = 0.0f;
+          if (valid) {
+            T::template axis<DERIV>(rk.x, tp, sx, wx, dx);
+            T::template axis<DERIV>(rk.y, tp, sy, wy, dy);
+            T::origin(rk.z, sz, dz0);
+          }
+          const int row0 = sx * G::SY + sy, col0 = sz + (G::ZLO - G::HLO);
+          if (!__any_sync(0xffffffffu, valid)) continue;  // warp-uniform
+          const int rot = skew_match((row0 * 8 + col0) & 31, valid);
+          if (!valid) continue;
+          T::template axis_skew<DERIV>(dz0, tp, rot, wU, wW, dU, dW);
+#pragma unroll
+          for (int j = 0; j < 8; ++j) nx[j] = (j + rot) >= 8 ? 1 : 0;
+          p0 = s_val + (row0 * G::PITCH + col0 + rot);
+        } else {
+          T::template axis<DERIV>(apply_shift<T>(rk.x, tp.frac[0]), tp, sx, wx, dx);
+          T::template axis<DERIV>(apply_shift<T>(rk.y, tp.frac[1]), tp, sy, wy, dy);
+          T::template axis<DERIV>(apply_shift<T>(rk.z, tp.frac[2]), tp, sz, wz, dz);
+        }
         // (TMA's 128-byte swizzle of the MAIN plane was measured: it is correct but RAISES the bank conflicts of
         // Lagrangian-ordered particles from 85 M to 136 M wavefronts, 1.09 -> 1.21 ms: with a row pitch of 32 words
         // lanes at distinct z already sit in distinct banks, and the swizzle scatters them.)
@@ -985,6 +1209,24 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
           float acc[NST];
 #pragma unroll
           for (int a = 0; a < NST; ++a) acc[a] = 0.0f;
+          if constexpr (T::SKEW) {
+#pragma unroll
+            for (int a = 0; a < P; ++a)
+#pragma unroll
+              for (int b = 0; b < P; ++b) {
+                const int a2 = b < P - 1 ? a : (a < P - 1 ? a + 1 : 0), b2 = b < P - 1 ? b + 1 : 0;
+                const int nextoff = skew_next_off<G>(a, b);
+                const float cur = wx[a] * wy[b], nxt = wx[a2] * wy[b2];
+                const float* rp = p0 + (a * G::SY + b) * G::PITCH;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  const float wgt = fmaf(nxt, wW[j], cur * wU[j]);
+                  const float* node = rp + (j + nx[j] * nextoff);
+#pragma unroll
+                  for (int q = 0; q < NST; ++q) acc[q] = fmaf(wgt, node[q * G::COMP], acc[q]);
+                }
+              }
+          } else {
 #pragma unroll
           for (int a = 0; a < P; ++a)
 #pragma unroll
@@ -998,6 +1240,7 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
                 for (int q = 0; q < NST; ++q) acc[q] = fmaf(wxyz, node[q * G::COMP], acc[q]);
               }
             }
+          }
           float* dst = out + (size_t)rk.w * NST;
           float nv[NST];
 #pragma unroll
@@ -1024,6 +1267,28 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
 #pragma unroll
           for (int a = 0; a < NST; ++a) coef[a] = a < gd.ncot ? __ldg(gd.cot + (size_t)rk.w * gd.cstride + a) : cc;
           float gx = 0.0f, gy = 0.0f, gz = 0.0f;
+          if constexpr (T::SKEW) {
+#pragma unroll
+            for (int a = 0; a < P; ++a)
+#pragma unroll
+              for (int b = 0; b < P; ++b) {
+                const int a2 = b < P - 1 ? a : (a < P - 1 ? a + 1 : 0), b2 = b < P - 1 ? b + 1 : 0;
+                const int nextoff = skew_next_off<G>(a, b);
+                const float cdx = dx[a] * wy[b], cdy = wx[a] * dy[b], cxy = wx[a] * wy[b];
+                const float ndx = dx[a2] * wy[b2], ndy = wx[a2] * dy[b2], nxy = wx[a2] * wy[b2];
+                const float* rp = p0 + (a * G::SY + b) * G::PITCH;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                  const float* node = rp + (j + nx[j] * nextoff);
+                  float val = 0.0f;
+#pragma unroll
+                  for (int q = 0; q < NST; ++q) val = fmaf(coef[q], node[q * G::COMP], val);
+                  gx = fmaf(fmaf(ndx, wW[j], cdx * wU[j]), val, gx);
+                  gy = fmaf(fmaf(ndy, wW[j], cdy * wU[j]), val, gy);
+                  gz = fmaf(fmaf(nxy, dW[j], cxy * dU[j]), val, gz);
+                }
+              }
+          } else {
 #pragma unroll
           for (int a = 0; a < P; ++a)
 #pragma unroll
@@ -1040,11 +1305,13 @@ __global__ void __launch_bounds__(BLOCK) k_gather(BinView bv, typename T::Params
                 gz = fmaf(wxy * dz[c], val, gz);
               }
             }
+          }
           float* dst = out + (size_t)rk.w * 3;
           dst[0] = out_scale != 0.0f ? fmaf(alpha, gx, out_scale * dst[0]) : alpha * gx;
           dst[1] = out_scale != 0.0f ? fmaf(alpha, gy, out_scale * dst[1]) : alpha * gy;
           dst[2] = out_scale != 0.0f ? fmaf(alpha, gz, out_scale * dst[2]) : alpha * gz;
         } else {  // JVP, Eq. C.13b: (t . d/du) W = tx dWx Wy Wz + ty Wx dWy Wz + tz Wx Wy dWz
+          static_assert(!T::SKEW || !JVP, "the forward-mode gather is not built for the ES kernel");
           float tx = 0.0f, ty = 0.0f, tz = 0.0f;
           if (gd.pos_tan) {
             const float* tp3 = gd.pos_tan + (size_t)rk.w * 3;
@@ -1192,8 +1459,8 @@ int run_gather(Ctx* c, const typename T::Params& tp, const int roll[3], const Ga
   const int m = c->mg;
   for (int a = 0; a < NST; ++a) {
     mp.p[a] = ga.mesh[a];
-    PM_TRY(make_mesh_tmap(c, ga.mesh[a], G::SX, G::SY, TZ, &maps.m[2 * a]));
-    PM_TRY(make_mesh_tmap(c, ga.mesh[a], G::SX, G::SY, G::HZ, &maps.m[2 * a + 1]));
+    PM_TRY(make_mesh_tmap(c, ga.mesh[a], G::SX, G::SY, G::DENSE ? G::PITCH : TZ, &maps.m[2 * a]));
+    PM_TRY(make_mesh_tmap(c, ga.mesh[a], G::SX, G::SY, G::HZ, &maps.m[2 * a + 1]));  // unused by DENSE tiles
   }
   const double inv_delta = (double)c->mg / c->p.box;
   GatherDev gd;

@@ -272,6 +272,22 @@ __global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? (XEPT >= 16 ? 3 : 2) 
   const float dyv = (float)t.grad[iy], dzv = (float)t.grad[iz];
   const double pcyz = t.pc[iy] * t.pc[iz] - t.ps[iy] * t.ps[iz], psyz = t.pc[iy] * t.ps[iz] + t.ps[iy] * t.pc[iz];
 
+  // NUFFT: the modes at or above the particle Nyquist are dropped (their window entry is 0, R8), which makes green_of
+  // zero along the whole line.  A CTA whose columns are all dropped -- three quarters of them at sigma = 2 -- has
+  // nothing to transform: its outputs are zero (cfg3: 7.5 -> 3.x ms for this kernel).
+  if (__syncthreads_and(!live || wyz == 0.0)) {
+    constexpr int NT = N * XC / XEPT;
+    const float2 zero = make_float2(0.f, 0.f);
+    if (live)
+      for (int p = tid / XC; p < N; p += NT / XC) {
+        const size_t o = (size_t)p * plane + q;
+        out0[o] = zero;
+        if (MODE == 0) out1[o] = zero, out2[o] = zero;
+        if (MODE == 1 && out1 != nullptr) out1[o] = zero;
+      }
+    return;
+  }
+
   // coeff / (Lap * window); 0 at n = 0 and for dropped modes.  The column part of the symbols is summed in fp64
   // once per thread; along the line everything is fp32 (the result is an fp32 factor anyway; the fp64 adds,
   // multiplies and the divide per mode were a quarter of the kernel's stall samples).

@@ -44,7 +44,7 @@ def _cuda_lib_dir(nvcc: str) -> str:
 
 def _units(es_widths=ES_WIDTHS, obj=OBJ):
     units = []
-    # widest kernels first: they take minutes to compile and should not start last
+    # widest kernels first: they take the longest to compile and should not start last
     for w in sorted(es_widths, reverse=True):
         for part in (2, 1, 0):
             units.append((os.path.join(CSRC, "nufft_mesh.cu"), os.path.join(obj, f"nufft_mesh_w{w}_p{part}.o"),

@@ -274,7 +274,7 @@ __global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? (XEPT >= 16 ? 3 : 2) 
 
   // NUFFT: the modes at or above the particle Nyquist are dropped (their window entry is 0, R8), which makes green_of
   // zero along the whole line.  A CTA whose columns are all dropped -- three quarters of them at sigma = 2 -- has
-  // nothing to transform: its outputs are zero (cfg3: 7.5 -> 3.x ms for this kernel).
+  // nothing to transform: its outputs are zero (cfg3: 7.5 -> 5.0 ms for this kernel).
   if (__syncthreads_and(!live || wyz == 0.0)) {
     constexpr int NT = N * XC / XEPT;
     const float2 zero = make_float2(0.f, 0.f);

@@ -232,6 +232,13 @@ int pm_sheet_resample(pm_ctx* ctx, const float* pos, int32_t n_p, int32_t r, flo
 /* Same as pm_force with HOST buffers: copies pos_host to the device, runs pm_force, copies the forces
  * back and synchronises.  Pinned host memory gives asynchronous copies; pageable memory also works. */
 int pm_force_host(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream);
+/* The same without the final synchronisation: the three steps are enqueued on `stream` and the call returns.  The
+ * host buffers must stay valid -- and must be pinned for the copies to be asynchronous -- until the caller has
+ * synchronised the stream.  One evaluation cannot overlap its own two copies (every force depends on every
+ * position), but two evaluations in flight can: with two ctx on two streams the device-to-host copy of one
+ * overlaps the host-to-device copy of the next and both directions of the host link stay busy (bench.py, e2e).
+ * The first call on a ctx allocates its staging buffers (and synchronises the device once). */
+int pm_force_host_async(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream);
 
 /* ---- measurement ------------------------------------------------------------------------------------ */
 /* When enabled, pm_force / pm_force_vjp record CUDA events around each stage on the caller's stream. */

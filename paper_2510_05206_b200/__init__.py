@@ -28,6 +28,7 @@ from .api import (  # noqa: F401
     pm_force,
     pm_force_vjp,
     pm_force_host,
+    pm_force_host_async,
     pm_assign_jvp,
     pm_interp_jvp,
     pm_dkd_step,

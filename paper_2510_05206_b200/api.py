@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = (
     "pm_interp", "pm_interp_vjp", "nufft_spread", "nufft_spread_vjp", "nufft_poisson_force",
     "nufft_poisson_force_vjp", "nufft_interp", "nufft_interp_vjp", "pm_force", "pm_force_vjp", "pm_force_host",
     "pm_set_profiling", "pm_get_stage_ms", "pm_assign_jvp", "pm_interp_jvp", "pm_dkd_step", "pm_dkd_step_adjoint",
-    "pm_power_spectrum", "pm_sheet_resample", "pm_smem_peak", "pm_mesh_power_noalloc",
+    "pm_power_spectrum", "pm_sheet_resample", "pm_smem_peak", "pm_mesh_power_noalloc", "pm_force_host_async",
 )
 
 STAGE_NAMES = ("bin", "assign", "fft_fwd", "kspace", "fft_inv", "interp", "vjp_scatter", "vjp_kspace", "vjp_gather",
@@ -109,6 +109,7 @@ def load_library(build_if_missing: bool = False):
         "pm_force": (C.c_int, [vp, vp, i64, vp, vp]),
         "pm_force_vjp": (C.c_int, [vp, vp, i64, vp, vp, vp]),
         "pm_force_host": (C.c_int, [vp, vp, i64, vp, vp]),
+        "pm_force_host_async": (C.c_int, [vp, vp, i64, vp, vp]),
         "pm_assign_jvp": (C.c_int, [vp, vp, vp, i64, f64p, vp, vp, vp, vp]),
         "pm_interp_jvp": (C.c_int, [vp, C.POINTER(vp), C.c_int, vp, i64, f64p, vp, C.POINTER(vp), vp, vp]),
         "pm_dkd_step": (C.c_int, [vp, vp, vp, i64, C.c_double, C.c_double, C.c_double, C.c_double, vp]),
@@ -411,6 +412,19 @@ def pm_force_host(ctx, pos_host, force_host):
         raise ValueError("force_host must have 3*N elements")
     ctx.check(load_library().pm_force_host(ctx.handle, pos_host.data_ptr(), n, force_host.data_ptr(), _stream()),
               "pm_force_host")
+
+
+def pm_force_host_async(ctx, pos_host, force_host):
+    """pm_force_host without the final synchronisation (enqueued on torch's current stream): the pinned host tensors
+    must stay alive and untouched until that stream has been synchronised."""
+    for t, name in ((pos_host, "pos_host"), (force_host, "force_host")):
+        if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+            raise TypeError(f"{name} must be a contiguous float32 CPU tensor")
+    n = _n(pos_host)
+    if force_host.numel() != 3 * n:
+        raise ValueError("force_host must have 3*N elements")
+    ctx.check(load_library().pm_force_host_async(ctx.handle, pos_host.data_ptr(), n, force_host.data_ptr(), _stream()),
+              "pm_force_host_async")
 
 
 def pm_smem_peak(ctx, kind: int) -> float:

@@ -523,7 +523,7 @@ int pm_sheet_resample(pm_ctx* ctx, const float* pos, int32_t n_p, int32_t r, flo
   return launch_sheet_resample(c, pos, n_p, r, pos_out, S(stream));
 }
 
-int pm_force_host(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream) {
+static int force_host_impl(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream, bool sync) {
   Ctx* c = C(ctx);
   if (!c) return PM_EINVAL;
   PM_TRY(enter_device(c));
@@ -546,8 +546,16 @@ int pm_force_host(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_ho
   PM_CUDA(c, cudaMemcpyAsync(c->host_pos_dev, pos_host, bytes, cudaMemcpyHostToDevice, st));
   PM_TRY(pm_force(ctx, c->host_pos_dev, N, c->host_force_dev, stream));
   PM_CUDA(c, cudaMemcpyAsync(force_host, c->host_force_dev, bytes, cudaMemcpyDeviceToHost, st));
-  PM_CUDA(c, cudaStreamSynchronize(st));
+  if (sync) PM_CUDA(c, cudaStreamSynchronize(st));
   return PM_OK;
+}
+
+int pm_force_host(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream) {
+  return force_host_impl(ctx, pos_host, N, force_host, stream, true);
+}
+
+int pm_force_host_async(pm_ctx* ctx, const float* pos_host, int64_t N, float* force_host, void* stream) {
+  return force_host_impl(ctx, pos_host, N, force_host, stream, false);
 }
 
 }  // extern "C"

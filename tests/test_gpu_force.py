@@ -268,6 +268,30 @@ def test_pm_force_host_matches_device(pm):
     pm.pm_destroy(ctx)
 
 
+def test_pm_force_host_async_two_in_flight(pm):
+    """pm_force_host_async on two ctx / two streams (the pipelined end-to-end mode of bench.py): different inputs in
+    flight at the same time, each result equal to the blocking call's and within the bar of the oracle."""
+    n_p = 48
+    posa, c = gen.make_config_positions("cfg1", n_p=n_p)
+    posb = np.ascontiguousarray(np.mod(posa[::-1] + np.float32(0.37 * c["box"] / c["m"]), np.float32(c["box"])))
+    n = posa.shape[0]
+    lanes = []
+    for pos in (posa, posb):
+        lanes.append((pm.pm_create(params_of(pm, c, n)), torch.from_numpy(pos).pin_memory(),
+                      torch.empty(n, 3).pin_memory(), torch.cuda.Stream()))
+    for _ in range(3):  # several rounds back to back on alternating streams
+        for ctx, ph, fh, st in lanes:
+            with torch.cuda.stream(st):
+                pm.pm_force_host_async(ctx, ph, fh)
+    torch.cuda.synchronize()
+    for (ctx, ph, fh, st), pos, tag in zip(lanes, (posa, posb), "ab"):
+        blocking = torch.empty(n, 3).pin_memory()
+        pm.pm_force_host(ctx, ph, blocking)
+        check(f"async_vs_blocking_{tag}", fh.numpy(), blocking.numpy(), 2e-6)
+        check(f"async_vs_oracle_{tag}", fh.numpy(), po.force(pos, c["m"], c["box"], **oracle_kw(c)), FORCE_TOL)
+        pm.pm_destroy(ctx)
+
+
 def test_run_to_run_spread(pm):
     """Atomics make the summation order, hence the fp32 result, vary from run to run.
     The fixed-point tile accumulators are order-independent, so only the global reductions on tile faces and cuFFT

@@ -60,6 +60,25 @@ template <int R, int SIGN>
 struct Dft;
 
 template <int SIGN>
+struct Dft<5, SIGN> {  // the upsampled NUFFT grids sigma = 5/4: m_f = 5 * 2^k
+  static __device__ __forceinline__ void run(float2 (&v)[5]) {
+    constexpr float c1 = 0.30901699437494742f, c2 = -0.80901699437494742f;  // cos(2 pi / 5), cos(4 pi / 5)
+    constexpr float s1 = 0.95105651629515357f, s2 = 0.58778525229247313f;   // sin(2 pi / 5), sin(4 pi / 5)
+    const float2 t1 = cadd(v[1], v[4]), t2 = cadd(v[2], v[3]), t3 = csub(v[1], v[4]), t4 = csub(v[2], v[3]);
+    const float2 x0 = v[0];
+    const float2 m1 = make_float2(x0.x + c1 * t1.x + c2 * t2.x, x0.y + c1 * t1.y + c2 * t2.y);
+    const float2 m2 = make_float2(x0.x + c2 * t1.x + c1 * t2.x, x0.y + c2 * t1.y + c1 * t2.y);
+    const float2 n1 = mul_i<SIGN>(make_float2(s1 * t3.x + s2 * t4.x, s1 * t3.y + s2 * t4.y));  // SIGN i (s1 t3 + s2 t4)
+    const float2 n2 = mul_i<SIGN>(make_float2(s2 * t3.x - s1 * t4.x, s2 * t3.y - s1 * t4.y));
+    v[0] = make_float2(x0.x + t1.x + t2.x, x0.y + t1.y + t2.y);
+    v[1] = cadd(m1, n1);
+    v[4] = csub(m1, n1);
+    v[2] = cadd(m2, n2);
+    v[3] = csub(m2, n2);
+  }
+};
+
+template <int SIGN>
 struct Dft<8, SIGN> {
   static __device__ __forceinline__ void run(float2 (&v)[8]) {
     // even / odd samples: X_k = E_k + W8^k O_k, X_{k+4} = E_k - W8^k O_k
@@ -130,6 +149,8 @@ template <> struct Radices<128>  { static constexpr int r0 = 16, r1 = 8,  r2 = 1
 template <> struct Radices<256>  { static constexpr int r0 = 16, r1 = 16, r2 = 1; };
 template <> struct Radices<512>  { static constexpr int r0 = 8,  r1 = 8,  r2 = 8; };
 template <> struct Radices<1024> { static constexpr int r0 = 16, r1 = 8,  r2 = 8; };
+template <> struct Radices<320>  { static constexpr int r0 = 5,  r1 = 8,  r2 = 8; };   // 5/4 * 256
+template <> struct Radices<640>  { static constexpr int r0 = 5,  r1 = 16, r2 = 8; };   // 5/4 * 512
 
 // One radix-R stage over sub-transforms of size S (M = S / R butterflies each).  tw[k] = e^{-2 pi i k / N}.
 //   forward (DIF): y = DFT_R(x), y_q *= W_S^{jq};      inverse (DIT): x_r *= conj(W_S)^{jr}, y = IDFT_R(x)
@@ -395,7 +416,9 @@ __global__ void __launch_bounds__(N* XC / XEPT, N <= 512 ? (XEPT >= 16 ? 3 : 2) 
 }
 
 // ---- host side -------------------------------------------------------------------------------------------
-bool xfft_supported(int m) { return m == 64 || m == 128 || m == 256 || m == 512 || m == 1024; }
+bool xfft_supported(int m) {
+  return m == 64 || m == 128 || m == 256 || m == 512 || m == 1024 || m == 320 || m == 640;
+}
 
 int xfft_init(Ctx* c) {  // twiddle table and the batched 2-D (y,z) cuFFT plans; called from pm_create
   c->xfused = false;
@@ -489,6 +512,8 @@ static int xfft_launch(Ctx* c, const float2* i0, const float2* i1, const float2*
     case 256: return xfft_launch_n<256, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
     case 512: return xfft_launch_n<512, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
     case 1024: return xfft_launch_n<1024, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
+    case 320: return xfft_launch_n<320, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
+    case 640: return xfft_launch_n<640, MODE>(c, t, i0, i1, i2, o0, o1, o2, coeff_eff, st);
   }
   return fail(c, PM_ESTATE, "fused x-FFT not built for m = %d", c->mg);
 }

@@ -137,10 +137,11 @@ def test_fused_kspace_plane_waves(pm, m, interlace):
     pm.pm_destroy(ctx)
 
 
-@pytest.mark.parametrize("m", [64, 128, 256, 512])
+@pytest.mark.parametrize("m", [64, 128, 256, 320, 512])
 def test_fused_kspace_random_mesh_vs_oracle(pm, m):
     """Every mode of the fused kernel against the oracle, element by element, on random meshes: forward and
-    transpose, interlaced (two input / two output meshes: the superset of the single-grid data flow)."""
+    transpose, interlaced (two input / two output meshes: the superset of the single-grid data flow).  m = 320 takes
+    the radix-5 first stage of the upsampled NUFFT grids (5/4 * 2^k)."""
     box = 500.0
     kw = dict(worder=3, grad_order=4, lap_order=0, deconv_pow=2, coeff=0.7)
     d = gen.random_mesh(m, 300 + m, 2)
@@ -304,12 +305,15 @@ def nufft_params(pm, m, box, n, sigma=2.0, eps=1e-6, width=0, flags=0):
                        grad_order=0, lap_order=0, flags=flags)
 
 
-@pytest.mark.parametrize("fine", [512, 1024])
-def test_nufft_kspace_plane_waves(pm, fine):
+@pytest.mark.parametrize("fine,sigma", [(512, 2.0), (1024, 2.0), (640, 1.25)])
+def test_nufft_kspace_plane_waves(pm, fine, sigma):
     """NUFFT Fourier-space stage on the fused kernel with the NUFFT tables (mode truncation, 1/phi_hat^2, i k / k^2)
-    at the cfg3 fine grid (1024) and at 512: closed form from the oracle's multiplier at single modes."""
-    m, box, npart = fine // 2, 1000.0, 12345
-    ctx = pm.pm_create(nufft_params(pm, m, box, 8))
+    at the cfg3 fine grid (1024), at 512 and at the paper-default setting of cfg3_paper (sigma = 5/4, w = 5, fine grid
+    640 = 5 * 128: radix-5 first stage): closed form from the oracle's multiplier at single modes."""
+    m, box, npart = int(round(fine / sigma)), 1000.0, 12345
+    ctx = pm.pm_create(nufft_params(pm, m, box, 8, sigma=sigma, eps=1e-6 if sigma == 2.0 else 1e-4,
+                                    width=0 if sigma == 2.0 else 5))
+    assert ctx.mg == fine
     w, beta = ctx.nufft_width, ctx.nufft_beta
     idx, c1 = gen.plane_wave_modes(fine, 600, 9200 + fine)
     # half of the modes inside the retained cube |n_a| < m/2, half anywhere (dropped: response 0)

@@ -435,7 +435,7 @@ def run_ours(args) -> int:
                                                       pos_c=(pos_np, c))}
         if not args.no_other_configs and not args.n_p:
             oc = {}
-            for name, vjp in (("cfg2", False), ("cfg4", True), ("cfg3", False), ("cfg3_paper", False)):
+            for name, vjp in (("cfg2", False), ("cfg4", True), ("cfg3", True), ("cfg3_paper", True)):
                 oc[name] = run_config(torch, pm, gen, name, rank, local, peak, 5, 3, vjp)
             extras["other_configs"] = oc
     if rank != 0:
